@@ -1,0 +1,63 @@
+/* ozfft.h -- C ABI of the emulated-fp64 FFT (arxiv/paper_2606_23698, "FP8 is All You Need, Part 2").
+ *
+ * The library computes the unnormalised complex DFT  Y_k = sum_j X_j w_N^{jk}, per axis of a
+ * 3-D array, as a Bailey six-step transform whose kernels contain no fp64
+ * arithmetic: Ozaki-II residue GEMMs on tcgen05 tensor cores (Alg. 1 at 216-241), tc-CRT
+ * reconstruction and Kulisch integer accumulation with a two-sided lift and one correctly
+ * rounded pack per stage output (Alg. 2).
+ *
+ * Conventions (readings S1..S8): sign = -1 forward (w_N = exp(-2 pi i/N)), +1 inverse, never
+ * normalised.  Sizes are powers of two, 2 <= n <= 1024 per axis.  Arrays are row-major, z fastest:
+ * element (x,y,z) at index (x*ny + y)*nz + z; one element = {re, im} as two IEEE-754 binary64 (16 bytes).
+ * `in` and `out` are DEVICE pointers, 16-byte aligned, must not overlap; `in` is read only, `out` is fully
+ * overwritten.  Inputs must be finite; a column holding a non-finite value produces NaN in the outputs of
+ * that 1-D transform stage.  All plan memory (tables, workspace) is owned by the plan; the caller owns in/out.
+ * ozfft_exec is asynchronous and ordered on `stream` (a cudaStream_t passed as void*); it never synchronises.
+ * A plan must not execute concurrently on two streams (it owns workspace).  No CPU fallback exists.
+ */
+#ifndef OZFFT_H
+#define OZFFT_H
+#include <stddef.h>
+#include <stdint.h>
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define OZFFT_OK 0
+#define OZFFT_EINVAL 1 /* null / misaligned pointer, bad size or sign, destroyed plan */
+#define OZFFT_ECUDA 2  /* CUDA allocation or launch failure; text in ozfft_last_error() */
+
+typedef struct ozfft_plan_s *ozfft_plan; /* opaque, library-owned */
+
+/* 3-D plan (three axis passes z, y, x).  NULL on failure. */
+ozfft_plan ozfft_plan_create(int nx, int ny, int nz, int sign);
+/* batched contiguous 1-D plan: `batch` pencils of length n, pencil b at element offset b*n (BASELINE.json
+ * config 3; one Bailey transform).  NULL on failure. */
+ozfft_plan ozfft_plan_create_1d(int n, int batch, int sign);
+/* out = DFT(in).  Device pointers to nx*ny*nz (or n*batch) complex128.  Returns OZFFT_*. */
+int ozfft_exec(ozfft_plan plan, const void *in, void *out, void *stream);
+/* Same through HOST buffers: copies in to the device, runs, copies back, synchronises `stream`. */
+int ozfft_exec_host(ozfft_plan plan, const void *host_in, void *host_out, void *stream);
+void ozfft_plan_destroy(ozfft_plan plan); /* NULL is a no-op */
+const char *ozfft_last_error(void);       /* thread-local text of the last failure */
+
+/* ---- introspection / test hooks (not needed by users) ---- */
+/* FNV-1a over the plan's 1024-entry table of (RN(2^53 cos), RN(2^53 sin)) of 2 pi t/1024 (reading S5);
+ * must equal the oracle's independent generator. */
+uint64_t ozfft_twiddle_checksum(void);
+/* Kernel launches one ozfft_exec of this plan issues. */
+int ozfft_plan_num_launches(ozfft_plan plan);
+/* Device bytes the plan owns (tables + workspace). */
+size_t ozfft_plan_device_bytes(ozfft_plan plan);
+/* Run only axis pass `axis` (0 = z, 1 = y, 2 = x; a 1-D plan has axis 0 only) of a 3-D plan: out = pass(in).
+ * Used by the sampled-pencil parity check at sizes the oracle cannot hold in full. */
+int ozfft_exec_axis(ozfft_plan plan, int axis, const void *in, void *out, void *stream);
+/* Silicon-contract probe: D[128][n] (raw 32-bit accumulators) = A[128][kbytes] * B[n][kbytes]^T as chained
+ * M=128 tcgen05.mma of K = 32 bytes each.  kind 0: f8f6f4 E4M3 -> f32; 1: f16 -> f32; 2: i8 (s8) -> s32;
+ * 3: f16 with A fed from TMEM.  All pointers device.  n multiple of 16 in [16,256], kbytes multiple of 32. */
+int ozfft_probe_mma(int kind, int n, int kbytes, const void *dA, const void *dB, void *dD, void *stream);
+
+#ifdef __cplusplus
+}
+#endif
+#endif

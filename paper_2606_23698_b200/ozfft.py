@@ -1,0 +1,131 @@
+"""Thin ctypes binding of libozfft.so (include/ozfft.h). Argument marshalling only.
+
+PyTorch supplies device memory and streams; every step of the transform runs in the CUDA kernels behind
+the C ABI. There is no CPU fallback: if the library is missing or fails, this raises.
+"""
+import ctypes as C
+import os
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SO = os.path.join(_HERE, "libozfft.so")
+_lib = None
+
+SYMBOLS = ["ozfft_plan_create", "ozfft_plan_create_1d", "ozfft_exec", "ozfft_exec_host", "ozfft_plan_destroy",
+           "ozfft_last_error", "ozfft_twiddle_checksum", "ozfft_plan_num_launches", "ozfft_plan_device_bytes",
+           "ozfft_exec_axis", "ozfft_probe_mma"]
+
+
+def lib():
+    global _lib
+    if _lib is None:
+        if not os.path.exists(_SO):
+            raise RuntimeError(f"{_SO} not built: run `python paper_2606_23698_b200/build.py` (no fallback path exists)")
+        L = C.CDLL(_SO)
+        vp = C.c_void_p
+        L.ozfft_plan_create.restype = vp
+        L.ozfft_plan_create.argtypes = [C.c_int] * 4
+        L.ozfft_plan_create_1d.restype = vp
+        L.ozfft_plan_create_1d.argtypes = [C.c_int] * 3
+        L.ozfft_exec.argtypes = [vp, vp, vp, vp]
+        L.ozfft_exec_host.argtypes = [vp, vp, vp, vp]
+        L.ozfft_exec_axis.argtypes = [vp, C.c_int, vp, vp, vp]
+        L.ozfft_plan_destroy.argtypes = [vp]
+        L.ozfft_plan_destroy.restype = None
+        L.ozfft_last_error.restype = C.c_char_p
+        L.ozfft_twiddle_checksum.restype = C.c_uint64
+        L.ozfft_plan_num_launches.argtypes = [vp]
+        L.ozfft_plan_device_bytes.argtypes = [vp]
+        L.ozfft_plan_device_bytes.restype = C.c_size_t
+        L.ozfft_probe_mma.argtypes = [C.c_int, C.c_int, C.c_int, vp, vp, vp, vp]
+        _lib = L
+    return _lib
+
+
+def last_error():
+    return lib().ozfft_last_error().decode()
+
+
+def _stream(stream):
+    if stream is not None:
+        return stream
+    import torch
+    return torch.cuda.current_stream().cuda_stream
+
+
+def _check(rc, what):
+    if rc != 0:
+        raise RuntimeError(f"{what} failed (code {rc}): {last_error()}")
+
+
+class Plan:
+    """ozfft plan. Plan(nx, ny, nz, sign=-1) for 3-D; Plan.batched_1d(n, batch, sign=-1) for contiguous pencils."""
+
+    def __init__(self, nx, ny, nz, sign=-1, _handle=None, _count=None):
+        self.h = _handle if _handle is not None else lib().ozfft_plan_create(nx, ny, nz, sign)
+        self.count = _count if _count is not None else nx * ny * nz
+        if not self.h:
+            raise RuntimeError("ozfft_plan_create failed: " + last_error())
+
+    @classmethod
+    def batched_1d(cls, n, batch, sign=-1):
+        h = lib().ozfft_plan_create_1d(n, batch, sign)
+        if not h:
+            raise RuntimeError("ozfft_plan_create_1d failed: " + last_error())
+        return cls(0, 0, 0, sign, _handle=h, _count=n * batch)
+
+    def _args(self, x, out):
+        import torch
+        assert x.is_cuda and x.dtype == torch.complex128 and x.is_contiguous() and x.numel() == self.count
+        if out is None:
+            out = torch.empty_like(x)
+        assert out.is_cuda and out.dtype == torch.complex128 and out.is_contiguous() and out.numel() == self.count
+        return x, out
+
+    def exec(self, x, out=None, stream=None):
+        """x, out: CUDA complex128 tensors (contiguous). Asynchronous on the stream."""
+        x, out = self._args(x, out)
+        _check(lib().ozfft_exec(self.h, x.data_ptr(), out.data_ptr(), _stream(stream)), "ozfft_exec")
+        return out
+
+    def exec_axis(self, axis, x, out=None, stream=None):
+        x, out = self._args(x, out)
+        _check(lib().ozfft_exec_axis(self.h, axis, x.data_ptr(), out.data_ptr(), _stream(stream)), "ozfft_exec_axis")
+        return out
+
+    def exec_host(self, x_host, out_host, stream=None):
+        """x_host, out_host: CPU complex128 tensors (pinned for speed). Synchronous."""
+        _check(lib().ozfft_exec_host(self.h, x_host.data_ptr(), out_host.data_ptr(), _stream(stream)), "ozfft_exec_host")
+        return out_host
+
+    @property
+    def num_launches(self):
+        return lib().ozfft_plan_num_launches(self.h)
+
+    @property
+    def device_bytes(self):
+        return lib().ozfft_plan_device_bytes(self.h)
+
+    def destroy(self):
+        if self.h:
+            lib().ozfft_plan_destroy(self.h)
+            self.h = None
+
+    def __del__(self):
+        try:
+            self.destroy()
+        except Exception:
+            pass
+
+
+def twiddle_checksum():
+    return int(lib().ozfft_twiddle_checksum())
+
+
+def probe_mma(kind, A, B):
+    """A: uint8 CUDA tensor [128, kbytes]; B: uint8 CUDA [n, kbytes] -> int32 CUDA [128, n] raw accumulators."""
+    import torch
+    n, kb = B.shape
+    D = torch.zeros((128, n), dtype=torch.int32, device=A.device)
+    _check(lib().ozfft_probe_mma(kind, n, kb, A.data_ptr(), B.data_ptr(), D.data_ptr(), _stream(None)), "ozfft_probe_mma")
+    torch.cuda.synchronize()
+    return D
