@@ -1,0 +1,345 @@
+// ozfft.cu -- plan, stage scheduling and the C ABI of include/ozfft.h.
+// Axis passes z, y, x; each axis is one stage (n <= 32) or two stages with the twiddle
+// fused into the second-stage matrices (Eq. 6).  The array between stages is
+// fp64 (one correctly rounded pack per stage output, Alg. 2 line 16).
+#include <cstdio>
+#include <cstdlib>
+#include <cstring>
+#include <map>
+#include <string>
+#include <vector>
+
+#include "ozfft.h"
+#include "stage.cuh"
+#include "stage_simt.cuh"
+#include "stage_tc.cuh"
+#include "tables.cuh"
+
+using namespace oz;
+
+namespace {
+
+thread_local std::string g_err = "";
+void set_err(const std::string &s) { g_err = s; }
+bool cuda_ok(cudaError_t e, const char *what) {
+    if (e == cudaSuccess) return true;
+    set_err(std::string(what) + ": " + cudaGetErrorString(e));
+    return false;
+}
+
+const Twiddles &twiddles() {
+    static Twiddles T;
+    static bool init = false;
+    if (!init) { build_twiddles(T); init = true; }
+    return T;
+}
+
+struct StageLaunch {
+    StageGeom g;
+    const ushort2 *mat_simt;  // [nmat][12][K][K] (a_R, a_I) canonical residues
+    const uint8_t *mat_tc;    // digit planes for the tensor-core kernel (stage_tc.cuh)
+    int axis;
+};
+
+}  // namespace
+
+struct ozfft_plan_s {
+    uint32_t magic;
+    int nx, ny, nz, sign;
+    long long count;
+    int variant;  // 0 simt, 1 tensor-core
+    std::vector<StageLaunch> stages;
+    std::vector<void *> dev_allocs;
+    size_t dev_bytes;
+    DevConsts *d_consts;
+    void *work;
+    void *h_in, *h_out;  // device staging for ozfft_exec_host (lazy)
+};
+
+namespace {
+
+constexpr uint32_t PLAN_MAGIC = 0x4F5A4646u;
+
+bool is_pow2(int n) { return n >= 2 && (n & (n - 1)) == 0; }
+
+void fill_consts(DevConsts &c) {
+    CrtConsts C;
+    build_crt(C);
+    for (int k = 0; k < R_MOD; k++) {
+        const uint32_t m = (uint32_t)kModuli[k];
+        c.m[k] = m;
+        c.mu[k] = (uint32_t)((1ull << 32) / m);
+        c.c16[k] = (uint32_t)((1ull << 16) % m);
+        c.c32[k] = (uint32_t)((1ull << 32) % m);
+        c.c48[k] = (uint32_t)((1ull << 48) % m);
+        c.off28[k] = (uint32_t)((((1u << 28) + m - 1) / m) * m);
+        for (int l = 0; l < 4; l++) c.u[k][l] = (uint32_t)(C.u[k] >> (32 * l));
+        c.wlo[k] = (uint32_t)C.w[k];
+        c.whi[k] = (uint32_t)(C.w[k] >> 32);
+    }
+    for (int l = 0; l < 4; l++) {
+        c.M[l] = (uint32_t)(C.M >> (32 * l));
+        c.Mh[l] = (uint32_t)(C.Mhalf >> (32 * l));
+    }
+}
+
+// table index t (into omega_1024) of matrix `mid`, row k, column j.  fusedN == 0: plain F_K;
+// else the twiddle-fused second-stage matrix of a length-fusedN transform for k2 = mid (Eq. 6).
+inline int tw_index(int K, int fusedN, int mid, int k, int j) {
+    if (!fusedN) return (int)(((long)(TABLE_N / K) * j * k) % TABLE_N);
+    return (int)(((long)(TABLE_N / fusedN) * j * (mid + 32L * k)) % TABLE_N);
+}
+
+struct MatKey {
+    int K, fusedN;
+    bool operator<(const MatKey &o) const { return K != o.K ? K < o.K : fusedN < o.fusedN; }
+};
+
+void *dev_upload(ozfft_plan_s *p, const void *src, size_t bytes) {
+    void *d = nullptr;
+    if (!cuda_ok(cudaMalloc(&d, bytes), "cudaMalloc(table)")) return nullptr;
+    if (!cuda_ok(cudaMemcpy(d, src, bytes, cudaMemcpyHostToDevice), "cudaMemcpy(table)")) { cudaFree(d); return nullptr; }
+    p->dev_allocs.push_back(d);
+    p->dev_bytes += bytes;
+    return d;
+}
+
+const ushort2 *build_mat_simt(ozfft_plan_s *p, int K, int fusedN) {
+    const Twiddles &T = twiddles();
+    const int nmat = fusedN ? 32 : 1;
+    std::vector<ushort2> h((size_t)nmat * 12 * K * K);
+    for (int mid = 0; mid < nmat; mid++)
+        for (int i = 0; i < 12; i++)
+            for (int k = 0; k < K; k++)
+                for (int j = 0; j < K; j++) {
+                    const int t = tw_index(K, fusedN, mid, k, j);
+                    ushort2 a;
+                    a.x = (unsigned short)residue_of(T.c[t], kModuli[i]);
+                    a.y = (unsigned short)residue_of((int64_t)p->sign * T.s[t], kModuli[i]);
+                    h[(((size_t)mid * 12 + i) * K + k) * K + j] = a;
+                }
+    return (const ushort2 *)dev_upload(p, h.data(), h.size() * sizeof(ushort2));
+}
+
+struct AxisDesc {
+    bool contiguous;
+    long long outer, N, inner;  // strided: element (o, i, z) at (o*N + i)*inner + z; contiguous: pencil P at P*N
+};
+
+bool add_axis(ozfft_plan_s *p, const AxisDesc &a, int axis, std::map<MatKey, std::pair<const ushort2 *, const uint8_t *>> &mats) {
+    const int N = (int)a.N;
+    const bool two = N > 32;
+    const int q = two ? 32 : N, pp = two ? N / 32 : 1;
+    auto get = [&](int K, int fusedN, StageLaunch &s) -> bool {
+        MatKey key{K, fusedN};
+        auto it = mats.find(key);
+        if (it == mats.end()) {
+            const ushort2 *ms = build_mat_simt(p, K, fusedN);
+            if (!ms) return false;
+            const uint8_t *mt = nullptr;
+            if (p->variant == 1) {
+                std::vector<uint8_t> h;
+                build_mat_tc(h, K, fusedN, p->sign, twiddles());
+                mt = (const uint8_t *)dev_upload(p, h.data(), h.size());
+                if (!mt) return false;
+            }
+            it = mats.insert({key, {ms, mt}}).first;
+        }
+        s.mat_simt = it->second.first;
+        s.mat_tc = it->second.second;
+        return true;
+    };
+    StageLaunch s1{}, s2{};
+    s1.axis = s2.axis = axis;
+    StageGeom &g1 = s1.g, &g2 = s2.g;
+    g1.K = q;
+    g1.nmat = 1;
+    g1.matsel = 0;
+    if (!a.contiguous) {
+        const long long I = a.inner;
+        g1.n0 = (int)(I / 32); g1.n1 = pp; g1.n2 = (int)a.outer;
+        g1.i0 = 32; g1.i1 = I; g1.i2 = a.N * I;
+        g1.lane = 1; g1.ji = pp * I; g1.ko = pp * I;
+        g2.K = pp; g2.n0 = (int)(I / 32); g2.n1 = 32; g2.n2 = (int)a.outer;
+        g2.i0 = 32; g2.i1 = pp * I; g2.i2 = a.N * I;
+        g2.o0 = 32; g2.o1 = I; g2.o2 = a.N * I;
+        g2.lane = 1; g2.ji = I; g2.ko = 32 * I; g2.matsel = 2;
+    } else {
+        const long long Pn = a.outer;
+        g1.n0 = pp; g1.n1 = (int)(Pn / 32); g1.n2 = 1;
+        g1.i0 = 1; g1.i1 = 32 * a.N; g1.i2 = 0;
+        g1.lane = a.N; g1.ji = pp; g1.ko = pp;
+        g2.K = pp; g2.n0 = 32; g2.n1 = (int)(Pn / 32); g2.n2 = 1;
+        g2.i0 = pp; g2.i1 = 32 * a.N; g2.i2 = 0;
+        g2.o0 = 1; g2.o1 = 32 * a.N; g2.o2 = 0;
+        g2.lane = a.N; g2.ji = 1; g2.ko = 32; g2.matsel = 1;
+    }
+    g1.o0 = g1.i0; g1.o1 = g1.i1; g1.o2 = g1.i2;
+    g2.nmat = 32;
+    if (!get(q, 0, s1)) return false;
+    p->stages.push_back(s1);
+    if (two) {
+        if (!get(pp, N, s2)) return false;
+        p->stages.push_back(s2);
+    }
+    return true;
+}
+
+int pick_variant() {
+    const char *v = getenv("OZFFT_VARIANT");
+    if (v && !strcmp(v, "tc")) return 1;
+    return 0;
+}
+
+ozfft_plan_s *make_plan(int nx, int ny, int nz, int sign, bool batched1d) {
+    if (sign != -1 && sign != 1) { set_err("sign must be -1 (forward) or +1 (inverse)"); return nullptr; }
+    int dev = 0;
+    cudaDeviceProp prop;
+    if (!cuda_ok(cudaGetDevice(&dev), "cudaGetDevice") || !cuda_ok(cudaGetDeviceProperties(&prop, dev), "cudaGetDeviceProperties"))
+        return nullptr;
+    if (prop.major != 10) { set_err("ozfft needs an sm_100 device (B200); no fallback path exists"); return nullptr; }
+    ozfft_plan_s *p = new ozfft_plan_s();
+    p->magic = PLAN_MAGIC;
+    p->nx = nx; p->ny = ny; p->nz = nz; p->sign = sign;
+    p->count = (long long)nx * ny * nz;
+    p->variant = pick_variant();
+    p->dev_bytes = 0;
+    p->work = p->h_in = p->h_out = nullptr;
+    DevConsts hc;
+    fill_consts(hc);
+    p->d_consts = (DevConsts *)dev_upload(p, &hc, sizeof(hc));
+    std::map<MatKey, std::pair<const ushort2 *, const uint8_t *>> mats;
+    bool ok = p->d_consts != nullptr;
+    if (batched1d) {  // nx = batch, nz = n
+        ok = ok && add_axis(p, AxisDesc{true, nx, nz, 1}, 0, mats);
+    } else {
+        ok = ok && add_axis(p, AxisDesc{true, (long long)nx * ny, nz, 1}, 0, mats);
+        ok = ok && add_axis(p, AxisDesc{false, nx, ny, nz}, 1, mats);
+        ok = ok && add_axis(p, AxisDesc{false, 1, nx, (long long)ny * nz}, 2, mats);
+    }
+    if (ok) {
+        ok = cuda_ok(cudaMalloc(&p->work, (size_t)p->count * 16), "cudaMalloc(workspace)");
+        if (ok) p->dev_bytes += (size_t)p->count * 16;
+    }
+    if (ok && p->variant == 1) ok = stage_tc_prepare();
+    if (!ok) {
+        std::string keep = g_err;
+        ozfft_plan_destroy(p);
+        set_err(keep);
+        return nullptr;
+    }
+    return p;
+}
+
+bool valid(ozfft_plan p) { return p && p->magic == PLAN_MAGIC; }
+
+int launch_stage(ozfft_plan p, const StageLaunch &s, const void *src, void *dst, cudaStream_t st) {
+    const long long nt = tile_count(s.g);
+    if (p->variant == 1) return stage_tc_launch(s.g, src, dst, s.mat_tc, p->d_consts, st) ? OZFFT_OK : OZFFT_ECUDA;
+    const size_t sm = (size_t)s.g.K * 32 * 16 + (size_t)12 * s.g.K * 32 * 4;
+    static bool attr = false;
+    if (!attr) {
+        cudaFuncSetAttribute(stage_simt_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 32 * 32 * 16 + 12 * 32 * 32 * 4);
+        attr = true;
+    }
+    stage_simt_kernel<<<(unsigned)nt, SIMT_THREADS, sm, st>>>(s.g, (const ulonglong2 *)src, (ulonglong2 *)dst, s.mat_simt, p->d_consts);
+    return cuda_ok(cudaGetLastError(), "stage_simt_kernel launch") ? OZFFT_OK : OZFFT_ECUDA;
+}
+
+// run stages [first, last) : src -> ... -> dst, alternating through the plan workspace so the last lands in dst
+int run_stages(ozfft_plan p, size_t first, size_t last, const void *in, void *out, cudaStream_t st) {
+    const size_t L = last - first;
+    const void *src = in;
+    for (size_t i = 0; i < L; i++) {
+        void *dst = ((L - 1 - i) & 1) ? p->work : out;
+        int rc = launch_stage(p, p->stages[first + i], src, dst, st);
+        if (rc) return rc;
+        src = dst;
+    }
+    return OZFFT_OK;
+}
+
+bool check_ptrs(const void *in, void *out) {
+    if (!in || !out || ((uintptr_t)in & 15) || ((uintptr_t)out & 15) || in == out) {
+        set_err("in/out must be distinct, non-null, 16-byte aligned device pointers");
+        return false;
+    }
+    return true;
+}
+
+}  // namespace
+
+extern "C" {
+
+ozfft_plan ozfft_plan_create(int nx, int ny, int nz, int sign) {
+    if (!is_pow2(nx) || !is_pow2(ny) || !is_pow2(nz) || nx > 1024 || ny > 1024 || nz > 1024) {
+        set_err("sizes must be powers of two in [2, 1024]");
+        return nullptr;
+    }
+    if (nz % 32 || ((long long)nx * ny) % 32) {
+        set_err("unsupported shape: nz and nx*ny must be multiples of 32 (tile width)");
+        return nullptr;
+    }
+    return make_plan(nx, ny, nz, sign, false);
+}
+
+ozfft_plan ozfft_plan_create_1d(int n, int batch, int sign) {
+    if (!is_pow2(n) || n > 1024 || batch < 32 || batch % 32) {
+        set_err("n must be a power of two in [2, 1024] and batch a positive multiple of 32");
+        return nullptr;
+    }
+    return make_plan(batch, 1, n, sign, true);
+}
+
+int ozfft_exec(ozfft_plan p, const void *in, void *out, void *stream) {
+    if (!valid(p)) { set_err("invalid or destroyed plan"); return OZFFT_EINVAL; }
+    if (!check_ptrs(in, out)) return OZFFT_EINVAL;
+    return run_stages(p, 0, p->stages.size(), in, out, (cudaStream_t)stream);
+}
+
+int ozfft_exec_axis(ozfft_plan p, int axis, const void *in, void *out, void *stream) {
+    if (!valid(p)) { set_err("invalid or destroyed plan"); return OZFFT_EINVAL; }
+    if (!check_ptrs(in, out)) return OZFFT_EINVAL;
+    size_t first = p->stages.size(), last = 0;
+    for (size_t i = 0; i < p->stages.size(); i++)
+        if (p->stages[i].axis == axis) { first = i < first ? i : first; last = i + 1; }
+    if (first >= last) { set_err("no such axis in this plan"); return OZFFT_EINVAL; }
+    return run_stages(p, first, last, in, out, (cudaStream_t)stream);
+}
+
+int ozfft_exec_host(ozfft_plan p, const void *host_in, void *host_out, void *stream) {
+    if (!valid(p)) { set_err("invalid or destroyed plan"); return OZFFT_EINVAL; }
+    if (!host_in || !host_out) { set_err("null host pointer"); return OZFFT_EINVAL; }
+    const size_t bytes = (size_t)p->count * 16;
+    if (!p->h_in) {
+        if (!cuda_ok(cudaMalloc(&p->h_in, bytes), "cudaMalloc(staging in)")) return OZFFT_ECUDA;
+        if (!cuda_ok(cudaMalloc(&p->h_out, bytes), "cudaMalloc(staging out)")) { cudaFree(p->h_in); p->h_in = nullptr; return OZFFT_ECUDA; }
+        p->dev_bytes += 2 * bytes;
+    }
+    cudaStream_t st = (cudaStream_t)stream;
+    if (!cuda_ok(cudaMemcpyAsync(p->h_in, host_in, bytes, cudaMemcpyHostToDevice, st), "H2D")) return OZFFT_ECUDA;
+    int rc = run_stages(p, 0, p->stages.size(), p->h_in, p->h_out, st);
+    if (rc) return rc;
+    if (!cuda_ok(cudaMemcpyAsync(host_out, p->h_out, bytes, cudaMemcpyDeviceToHost, st), "D2H")) return OZFFT_ECUDA;
+    return cuda_ok(cudaStreamSynchronize(st), "cudaStreamSynchronize") ? OZFFT_OK : OZFFT_ECUDA;
+}
+
+void ozfft_plan_destroy(ozfft_plan p) {
+    if (!valid(p)) return;
+    for (void *d : p->dev_allocs) cudaFree(d);
+    if (p->work) cudaFree(p->work);
+    if (p->h_in) cudaFree(p->h_in);
+    if (p->h_out) cudaFree(p->h_out);
+    p->magic = 0;
+    delete p;
+}
+
+const char *ozfft_last_error(void) { return g_err.c_str(); }
+
+uint64_t ozfft_twiddle_checksum(void) { return twiddle_fnv(twiddles()); }
+
+int ozfft_plan_num_launches(ozfft_plan p) { return valid(p) ? (int)p->stages.size() : -1; }
+
+size_t ozfft_plan_device_bytes(ozfft_plan p) { return valid(p) ? p->dev_bytes : 0; }
+
+}  // extern "C"

@@ -1,0 +1,103 @@
+// stage_simt.cuh -- all-SIMT stage kernel: the simplest correct form of one Bailey stage, kept as the
+// in-library cross-check for the tensor-core kernel (selected with OZFFT_VARIANT=simt).
+// Steps (Alg. 1, 220-241): load -> column exponent -> quantise -> residues mod m_i ->
+// residue DFT (direct 4-product complex form, IMAD) -> canonicalise -> exact CRT + lift -> pack.
+#pragma once
+#include "arith.cuh"
+#include "stage.cuh"
+
+namespace oz {
+
+constexpr int SIMT_THREADS = 256;
+constexpr int SIMT_KG = SIMT_THREADS / 32;
+
+// dynamic smem: bits[K][32] (16 B each) | xres[12][K][32] ushort2
+__global__ void __launch_bounds__(SIMT_THREADS) stage_simt_kernel(StageGeom g, const ulonglong2 *__restrict__ in,
+                                                                  ulonglong2 *__restrict__ out,
+                                                                  const ushort2 *__restrict__ mat,
+                                                                  const DevConsts *__restrict__ cptr) {
+    extern __shared__ __align__(16) uint8_t smem_raw[];
+    __shared__ int s_tmax[32];
+    __shared__ int s_flag[32];  // bit0: some nonzero finite, bit1: non-finite
+    __shared__ DevConsts c;
+    const int K = g.K;
+    ulonglong2 *s_bits = (ulonglong2 *)smem_raw;
+    ushort2 *s_x = (ushort2 *)(smem_raw + (size_t)K * 32 * 16);
+    const int tid = threadIdx.x, lane = tid & 31, grp = tid >> 5;
+
+    for (int i = tid; i < (int)(sizeof(DevConsts) / 4); i += SIMT_THREADS) ((uint32_t *)&c)[i] = ((const uint32_t *)cptr)[i];
+    if (tid < 32) { s_tmax[tid] = -100000; s_flag[tid] = 0; }
+    __syncthreads();
+
+    long long t = blockIdx.x;
+    const int t0 = (int)(t % g.n0);
+    t /= g.n0;
+    const int t1 = (int)(t % g.n1);
+    const int t2 = (int)(t / g.n1);
+    const long long ibase = t0 * g.i0 + t1 * g.i1 + t2 * g.i2 + lane * g.lane;
+    const long long obase = t0 * g.o0 + t1 * g.o1 + t2 * g.o2 + lane * g.lane;
+    const int mid = g.matsel == 1 ? t0 : (g.matsel == 2 ? t1 : 0);
+
+    // ---- load + column exponent (a1, a2)
+    for (int j = grp; j < K; j += SIMT_KG) {
+        const ulonglong2 v = in[ibase + j * g.ji];
+        s_bits[j * 32 + lane] = v;
+        int T, cls, fl = 0, tm = -100000;
+        cls = classify_top(v.x, T);
+        if (cls == CLS_FINITE) { fl |= 1; tm = T; }
+        if (cls == CLS_NONFINITE) fl |= 2;
+        cls = classify_top(v.y, T);
+        if (cls == CLS_FINITE) { fl |= 1; tm = max(tm, T); }
+        if (cls == CLS_NONFINITE) fl |= 2;
+        if (fl & 1) atomicMax(&s_tmax[lane], tm);
+        if (fl) atomicOr(&s_flag[lane], fl);
+    }
+    __syncthreads();
+    const int Tmax = s_tmax[lane], flag = s_flag[lane];
+
+    // ---- quantise + residues (a3)
+    for (int j = grp; j < K; j += SIMT_KG) {
+        const ulonglong2 v = s_bits[j * 32 + lane];
+        const uint64_t ar = (flag == 1) ? quantise_mag(v.x, Tmax) : 0, ai = (flag == 1) ? quantise_mag(v.y, Tmax) : 0;
+        const bool nr = v.x >> 63, ni = v.y >> 63;
+#pragma unroll
+        for (int i = 0; i < 12; i++) {
+            uint32_t rr = residue53(ar, i, c), ri = residue53(ai, i, c);
+            if (nr && rr) rr = c.m[i] - rr;
+            if (ni && ri) ri = c.m[i] - ri;
+            s_x[(i * K + j) * 32 + lane] = make_ushort2((unsigned short)rr, (unsigned short)ri);
+        }
+    }
+    __syncthreads();
+
+    // ---- residue DFT + reconstruction, one (column, k) per thread iteration (a4-a9)
+    const int gexp = 53 + 52 - Tmax;
+    for (int k = grp; k < K; k += SIMT_KG) {
+        ulonglong2 y;
+        if (flag & 2) {
+            y.x = y.y = 0x7FF8000000000000ull;
+        } else if (flag == 0) {
+            y.x = y.y = 0;
+        } else {
+            uint32_t vr[12], vi[12];
+#pragma unroll
+            for (int i = 0; i < 12; i++) {
+                const ushort2 *arow = mat + (((size_t)mid * 12 + i) * K + k) * K;
+                int re = 0, im = 0;
+                for (int j = 0; j < K; j++) {
+                    const ushort2 a = __ldg(arow + j);
+                    const ushort2 x = s_x[(i * K + j) * 32 + lane];
+                    re += (int)a.x * (int)x.x - (int)a.y * (int)x.y;
+                    im += (int)a.x * (int)x.y + (int)a.y * (int)x.x;
+                }
+                vr[i] = barrett((uint32_t)(re + (int)c.off28[i]), c.m[i], c.mu[i]);
+                vi[i] = barrett((uint32_t)(im + (int)c.off28[i]), c.m[i], c.mu[i]);
+            }
+            y.x = pack_rne(crt_centre(vr, c), gexp);
+            y.y = pack_rne(crt_centre(vi, c), gexp);
+        }
+        out[obase + k * g.ko] = y;
+    }
+}
+
+}  // namespace oz

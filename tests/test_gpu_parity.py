@@ -1,0 +1,155 @@
+"""GPU parity: the CUDA path (through the C ABI) against the CPU oracle, bit for bit (north_star: "the GPU
+result must be bit-exact against the oracle, because the only rounding is the final conversion")."""
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+TOL_F128 = 5e-15  # north_star: normwise relative error vs the __float128 naive DFT
+
+
+def _torch():
+    import torch
+    assert torch.cuda.is_available()
+    return torch
+
+
+def _run3d(x, sign=-1):
+    torch = _torch()
+    from paper_2606_23698_b200 import ozfft
+    plan = ozfft.Plan(*x.shape, sign=sign)
+    d = torch.from_numpy(x).cuda()
+    y = plan.exec(d)
+    torch.cuda.synchronize()
+    out = y.cpu().numpy()
+    plan.destroy()
+    return out
+
+
+def _run1d(x, sign=-1):
+    torch = _torch()
+    from paper_2606_23698_b200 import ozfft
+    batch, n = x.shape
+    plan = ozfft.Plan.batched_1d(n, batch, sign=sign)
+    y = plan.exec(torch.from_numpy(x).cuda())
+    torch.cuda.synchronize()
+    out = y.cpu().numpy()
+    plan.destroy()
+    return out
+
+
+def _bits(a):
+    return np.ascontiguousarray(a).view(np.uint64)
+
+
+def _assert_bit_exact(got, want):
+    gb, wb = _bits(got), _bits(want)
+    bad = np.flatnonzero(gb != wb)
+    assert bad.size == 0, f"{bad.size} of {gb.size} words differ; first at {bad[:5]}: got {gb.flat[bad[0]]:#x} want {wb.flat[bad[0]]:#x}"
+
+
+def test_config1_32cubed_bit_exact_and_accurate(O):
+    from paper_2606_23698_b200 import inputs
+    x = inputs.uniform_pm1((32, 32, 32), 0)
+    got = _run3d(x)
+    want, bad = O.fft3d(x, -1, route=0)
+    assert bad == 0
+    _assert_bit_exact(got, want)
+    idx = np.arange(0, 32 ** 3, 37, dtype=np.int64)
+    assert O.relerr_3d_f128(x, idx, got.reshape(-1)[idx]) <= TOL_F128
+
+
+def test_config2_128cubed_lograng_bit_exact(O):
+    from paper_2606_23698_b200 import inputs
+    x = inputs.loguniform((128, 128, 128), 1)
+    got = _run3d(x)
+    O.reset_capacity_violations()
+    want, _ = O.fft3d(x, -1, route=0)
+    assert O.capacity_violations() == 0
+    _assert_bit_exact(got, want)
+    rng = np.random.default_rng(5)
+    idx = np.sort(rng.choice(128 ** 3, 256, replace=False)).astype(np.int64)
+    assert O.relerr_3d_f128(x, idx, got.reshape(-1)[idx]) <= TOL_F128
+
+
+@pytest.mark.parametrize("shape", [(32, 64, 128), (64, 32, 32), (32, 32, 256), (2, 16, 32), (32, 4, 64)])
+def test_mixed_shapes_bit_exact(O, shape):
+    from paper_2606_23698_b200 import inputs
+    x = inputs.uniform_pm1(shape, 11)
+    _assert_bit_exact(_run3d(x), O.fft3d(x, -1, route=0)[0])
+
+
+def test_inverse_and_roundtrip(O):
+    from paper_2606_23698_b200 import inputs
+    x = inputs.uniform_pm1((32, 64, 64), 12)
+    y = _run3d(x, -1)
+    z = _run3d(y, +1)
+    _assert_bit_exact(z, O.fft3d(y, +1, route=0)[0])
+    assert np.linalg.norm(z / x.size - x) / np.linalg.norm(x) < 5e-15
+
+
+@pytest.mark.parametrize("n", [1024, 512, 64, 32, 8])
+def test_batched_1d_bit_exact(O, n):
+    from paper_2606_23698_b200 import inputs
+    x = inputs.normal((96, n), 2)
+    got = _run1d(x)
+    _assert_bit_exact(got, O.fft1d(x, -1, route=0)[0])
+    assert O.relerr_1d_f128(x[:8], got[:8]) <= TOL_F128
+
+
+def test_edge_columns_zero_subnormal_huge(O):
+    """all-zero columns, subnormal inputs, values near overflow, exact ties in the quantiser."""
+    rng = np.random.default_rng(3)
+    x = (rng.standard_normal((64, 1024)) + 1j * rng.standard_normal((64, 1024)))
+    x[0] = 0
+    x[1] *= 5e-324 * 1e3           # subnormal pencil
+    x[2] *= 1e300                  # outputs overflow-free but large
+    x[3, ::2] = 0
+    x[4] = 1.0                     # DC: exact closed form
+    x[5] = 0; x[5, 0] = 1.0        # impulse
+    x[6].real = np.ldexp(1.0, -rng.integers(0, 60, 1024)) * (1 + 2.0 ** -52)
+    x[7] = np.ldexp(x[7], rng.integers(-500, 500, 1024))
+    got = _run1d(x)
+    want = O.fft1d(x, -1, route=0)[0]
+    _assert_bit_exact(got, want)
+    assert got[4, 0] == 1024 and np.all(got[4, 1:] == 0)
+    assert np.all(got[5] == 1.0)
+
+
+def test_nonfinite_column_gives_nan(O):
+    x = np.ones((32, 64), dtype=np.complex128)
+    x[3, 5] = np.inf
+    got = _run1d(x)
+    assert np.isnan(got[3]).any()
+    _assert_bit_exact(got, O.fft1d(x, -1, route=0)[0])
+
+
+def test_exec_host_and_axis(O):
+    torch = _torch()
+    from paper_2606_23698_b200 import inputs, ozfft
+    x = inputs.uniform_pm1((32, 64, 32), 13)
+    plan = ozfft.Plan(32, 64, 32)
+    xin = torch.from_numpy(x).pin_memory()
+    out = torch.empty_like(xin).pin_memory()
+    plan.exec_host(xin, out)
+    _assert_bit_exact(out.numpy(), O.fft3d(x, -1, route=0)[0])
+    # one axis pass (y): every y-pencil equals the oracle's 1-D transform
+    ya = plan.exec_axis(1, torch.from_numpy(x).cuda()).cpu().numpy()
+    for (ix, iz) in [(0, 0), (7, 31), (31, 5)]:
+        _assert_bit_exact(ya[ix, :, iz], O.fft1d_pencil(x[ix, :, iz]))
+    assert plan.num_launches == 4 and plan.device_bytes > x.nbytes
+    plan.destroy()
+
+
+def test_bad_arguments():
+    torch = _torch()
+    from paper_2606_23698_b200 import ozfft
+    with pytest.raises(RuntimeError):
+        ozfft.Plan(32, 32, 48)
+    with pytest.raises(RuntimeError):
+        ozfft.Plan(32, 32, 16)  # nz not a multiple of the tile width
+    plan = ozfft.Plan(32, 32, 32)
+    x = torch.zeros(32 ** 3, dtype=torch.complex128, device="cuda")
+    assert ozfft.lib().ozfft_exec(plan.h, x.data_ptr(), x.data_ptr(), None) == 1  # in == out
+    assert ozfft.lib().ozfft_exec(plan.h, x.data_ptr() + 8, x.data_ptr(), None) == 1  # misaligned
+    plan.destroy()
