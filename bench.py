@@ -1,0 +1,284 @@
+#!/usr/bin/env python
+"""bench.py -- emulated-fp64 3-D FFT (arxiv/paper_2606_23698 hot path) on B200, one JSON line.
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--size 1024] [--impl ours|reference]
+
+A step is one forward complex128 3-D transform of size^3 (BASELINE.json configs[4] workload; size 1024 by
+default) through the C ABI (ozfft_exec): every stage of the hot path runs in the CUDA kernels.
+value = 5*N_tot*log2(N_tot) GFLOP/s (PAPER.md:859 flop convention) with the input resident in HBM;
+e2e = the same through ozfft_exec_host with pinned HOST buffers (H2D + D2H inside the timed region).
+N > 1 runs N independent replicas (one per rank, no collective: north_star fixes the path to one GPU;
+DESIGN.md "replicas only"), value = aggregate over ranks / max time.
+--impl reference times the CPU oracle (oracle/, plain C, OpenMP) on a bounded sample of the same workload.
+"""
+import argparse
+import json
+import math
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+SEED = 4  # BASELINE.json configs[4]
+
+
+def flops(n_tot):
+    return 5.0 * n_tot * math.log2(n_tot)
+
+
+def peaks():
+    try:
+        p = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
+        return float(p["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    except Exception:
+        return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+class ClockSampler:
+    """nvidia-smi clocks and throttle reasons sampled DURING the timed region (B200_PROFILING.md)."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.rows, self.proc, self.index = [], None, index
+
+    def __enter__(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q,
+                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.t = threading.Thread(target=self._read, daemon=True)
+            self.t.start()
+        except Exception:
+            self.proc = None
+        return self
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([c.strip() for c in line.split(",")])
+
+    def __exit__(self, *a):
+        if self.proc:
+            self.proc.terminate()
+            try:
+                self.proc.wait(timeout=5)
+            except Exception:
+                self.proc.kill()
+
+    def summary(self):
+        sm, mx, reasons = [], 0, set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in self.rows:
+            try:
+                sm.append(float(r[0]))
+                mx = max(mx, float(r[1]))
+                for n, v in zip(names, r[3:7]):
+                    if v.lower().startswith("active"):
+                        reasons.add(n)
+            except Exception:
+                pass
+        sm.sort()
+        return {"sm_mhz": sm[len(sm) // 2] if sm else None, "sm_max_mhz": mx or None, "reasons": sorted(reasons),
+                "samples": len(sm)}
+
+
+def cpu_oracle_sample(size, pencils):
+    """Times the oracle (as it stands, direct exact-integer route) on `pencils` length-`size` pencils of the
+    workload's own data; returns (seconds, threads)."""
+    from oracle import oracle
+    from paper_2606_23698_b200 import inputs
+    import numpy as np
+    x = (2.0 * inputs.uniform01(SEED, 0, 2 * pencils * size) - 1.0).view(np.complex128).reshape(pencils, size)
+    oracle.fft1d(x[:64], -1, route=0)  # page in
+    t = time.perf_counter()
+    oracle.fft1d(x, -1, route=0)
+    return time.perf_counter() - t, oracle.num_threads()
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    size = args.size
+    n_tot = size ** 3
+    pencils = 16384
+    total_pencils = 3 * size * size
+    times = []
+    threads = 1
+    for i in range(args.warmup + args.steps):
+        dt, threads = cpu_oracle_sample(size, pencils)
+        if i >= args.warmup:
+            times.append(dt)
+    t_step = sum(times) / len(times)
+    t_full = t_step * total_pencils / pencils  # extrapolated time of one whole transform
+    val = flops(n_tot) / t_full / 1e9
+    sample = f"{pencils} of {total_pencils} length-{size} pencils per step ({pencils / total_pencils:.4%} of one transform), extrapolated"
+    line = {"impl": "reference", "metric": "emulated_fp64_fft3d_gflops_5NlogN", "value": val, "unit": "GFLOP/s",
+            "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup, "ms_per_step": t_full * 1e3,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "int128", "data": "synthetic",
+            "config": {"workload": f"forward 3-D FFT {size}^3 complex128, uniform[-1,1), seed {SEED}"},
+            "cpu_baseline": {"value": val, "unit": "GFLOP/s", "cores": threads, "kind": "oracle", "sample": sample},
+            "e2e": {"value": val, "unit": "GFLOP/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line))
+
+
+def run_ours(args):
+    import numpy as np
+    import torch
+    import torch.distributed as dist
+    from paper_2606_23698_b200 import inputs, ozfft
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a B200: there is no CPU fallback")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    size = args.size
+    n_tot = size ** 3
+    shape = (size, size, size)
+    nbytes = 16 * n_tot
+
+    # synthetic input (configs[4] recipe), generated on the host in pinned memory, rank-specific seed offset
+    h_in = torch.empty(shape, dtype=torch.complex128).pin_memory()
+    inputs.uniform_pm1(shape, SEED + 1000 * rank, out=h_in.numpy())
+    h_out = torch.empty(shape, dtype=torch.complex128).pin_memory()
+    d_in = h_in.cuda()
+    d_out = torch.empty_like(d_in)
+    plan = ozfft.Plan(size, size, size, sign=-1)
+    launches = plan.num_launches
+    stream = torch.cuda.current_stream()
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for _ in range(args.warmup):
+        plan.exec(d_in, d_out)
+    barrier()
+    ev = [torch.cuda.Event(enable_timing=True) for _ in range(args.steps + 1)]
+    with ClockSampler(local) as cs:
+        ev[0].record(stream)
+        for i in range(args.steps):
+            plan.exec(d_in, d_out)
+            ev[i + 1].record(stream)
+        barrier()
+    ms = [ev[i].elapsed_time(ev[i + 1]) for i in range(args.steps)]
+    ms_step = sum(ms) / len(ms)
+    clocks = cs.summary()
+
+    # end to end through the public API with HOST buffers
+    e2e_steps = max(1, min(args.steps, 3))
+    plan.exec_host(h_in, h_out)  # warm-up (allocates the staging buffers)
+    barrier()
+    t0 = time.perf_counter()
+    for _ in range(e2e_steps):
+        plan.exec_host(h_in, h_out)
+    barrier()
+    e2e_ms = (time.perf_counter() - t0) * 1e3 / e2e_steps
+
+    # sanity inside the bench: device-resident and host paths agree bit for bit; round trip
+    same = bool(torch.equal(d_out.cpu().view(torch.float64), h_out.view(torch.float64)))
+    inv = ozfft.Plan(size, size, size, sign=+1)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record(stream)
+    inv.exec(d_out, d_in)  # overwrites d_in with the unnormalised round trip
+    e1.record(stream)
+    torch.cuda.synchronize()
+    inv_ms = e0.elapsed_time(e1)
+    chunk = 1 << 24
+    flat_rt, flat_x = d_in.view(-1), h_in.view(-1)
+    num = den = 0.0
+    for s in range(0, min(n_tot, 1 << 27), chunk):
+        a = flat_rt[s:s + chunk] / n_tot
+        b = flat_x[s:s + chunk].cuda()
+        num += float(((a - b).abs() ** 2).sum())
+        den += float((b.abs() ** 2).sum())
+    roundtrip = math.sqrt(num / den)
+    inv.destroy()
+
+    # cuFFT Z2Z context number (not part of the path)
+    cufft_ms = None
+    try:
+        d_in.copy_(h_in, non_blocking=False)
+        for _ in range(2):
+            y = torch.fft.fftn(d_in)
+            del y
+        torch.cuda.synchronize()
+        e0.record(stream)
+        y = torch.fft.fftn(d_in)
+        e1.record(stream)
+        torch.cuda.synchronize()
+        cufft_ms = e0.elapsed_time(e1)
+        del y
+    except Exception as ex:  # out of memory at the largest size is not fatal for the bench line
+        cufft_ms = None
+
+    t_max = torch.tensor([ms_step, e2e_ms], dtype=torch.float64, device="cuda")
+    if world > 1:
+        dist.all_reduce(t_max, op=dist.ReduceOp.MAX)
+    ms_step_max, e2e_ms_max = float(t_max[0]), float(t_max[1])
+
+    if rank == 0:
+        peak, peak_src = peaks()
+        alg_bytes_launch = 32.0 * n_tot  # 16 B read + 16 B write per element per stage launch
+        launch_ms = ms_step / launches
+        achieved = alg_bytes_launch / (launch_ms * 1e-3) / 1e9
+        line = {
+            "metric": "emulated_fp64_fft3d_gflops_5NlogN", "value": world * flops(n_tot) / (ms_step_max * 1e-3) / 1e9,
+            "unit": "GFLOP/s", "n_gpus": world, "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms_step_max,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "int32", "data": "synthetic",
+            "config": {"workload": f"forward 3-D FFT {size}^3 complex128, uniform[-1,1), seed {SEED} (BASELINE.json configs[4])",
+                       "parallelism": "replicas only" if world > 1 else "single GPU", "l2": "inputs_exceed_l2" if nbytes > (126 << 20) else "l2_resident",
+                       "variant": os.environ.get("OZFFT_VARIANT", "default"), "stage_launches_per_transform": launches},
+            "ms_per_transform": ms_step_max, "ms_per_transform_min": min(ms), "inverse_ms": inv_ms,
+            "roundtrip_rel_err": roundtrip, "host_and_device_paths_bit_identical": same,
+            "hbm_roof": {"alg_bytes": 96.0 * n_tot if launches == 6 else alg_bytes_launch * launches / 2,
+                         "roof_ms_at_measured_peak": 96.0 * n_tot / (peak * 1e9) * 1e3, "frac_of_roof": (96.0 * n_tot / (peak * 1e9) * 1e3) / ms_step},
+            "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+                         "traffic": None, "kernel": "stage kernel (all launches of a transform are this kernel)",
+                         "peak_source": peak_src, "alg_bytes_per_launch": alg_bytes_launch, "launch_ms": launch_ms},
+            "clocks": clocks,
+            "e2e": {"value": world * flops(n_tot) / (e2e_ms_max * 1e-3) / 1e9, "unit": "GFLOP/s", "ms": e2e_ms_max,
+                    "h2d_bytes_per_step": nbytes, "d2h_bytes_per_step": nbytes, "steps": e2e_steps},
+            "gpu_launches": launches * args.steps,
+            "context": {"cufft_z2z_ms": cufft_ms, "paper_projection_ms_B300": [63, 87], "paper_projection_ms_B200": [70, 96],
+                        "paper_hbm_roof_ms": 12.9},
+        }
+        if not args.no_cpu:
+            pencils = 16384
+            dt, threads = cpu_oracle_sample(size, pencils)
+            t_full = dt * (3 * size * size) / pencils
+            line["cpu_baseline"] = {"value": flops(n_tot) / t_full / 1e9, "unit": "GFLOP/s", "cores": threads, "kind": "oracle",
+                                    "sample": f"{pencils} of {3 * size * size} length-{size} pencils ({dt:.1f} s), extrapolated to one transform = {t_full:.0f} s"}
+        print(json.dumps(line))
+    plan.destroy()
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--size", type=int, default=1024)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg (profiling runs)")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()
