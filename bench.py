@@ -105,7 +105,7 @@ def run_reference(args):
         return
     size = args.size
     n_tot = size ** 3
-    pencils = 16384
+    pencils = 262144
     total_pencils = 3 * size * size
     times = []
     threads = 1
@@ -238,7 +238,7 @@ def run_ours(args):
             "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "int32", "data": "synthetic",
             "config": {"workload": f"forward 3-D FFT {size}^3 complex128, uniform[-1,1), seed {SEED} (BASELINE.json configs[4])",
                        "parallelism": "replicas only" if world > 1 else "single GPU", "l2": "inputs_exceed_l2" if nbytes > (126 << 20) else "l2_resident",
-                       "variant": os.environ.get("OZFFT_VARIANT", "default"), "stage_launches_per_transform": launches},
+                       "variant": os.environ.get("OZFFT_VARIANT", "tc"), "stage_launches_per_transform": launches},
             "ms_per_transform": ms_step_max, "ms_per_transform_min": min(ms), "inverse_ms": inv_ms,
             "roundtrip_rel_err": roundtrip, "host_and_device_paths_bit_identical": same,
             "hbm_roof": {"alg_bytes": 96.0 * n_tot if launches == 6 else alg_bytes_launch * launches / 2,
@@ -254,7 +254,7 @@ def run_ours(args):
                         "paper_hbm_roof_ms": 12.9},
         }
         if not args.no_cpu:
-            pencils = 16384
+            pencils = 262144
             dt, threads = cpu_oracle_sample(size, pencils)
             t_full = dt * (3 * size * size) / pencils
             line["cpu_baseline"] = {"value": flops(n_tot) / t_full / 1e9, "unit": "GFLOP/s", "cores": threads, "kind": "oracle",

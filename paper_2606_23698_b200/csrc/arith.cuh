@@ -16,6 +16,7 @@ struct DevConsts {
     uint32_t c32[12];    // 2^32 mod m
     uint32_t c48[12];    // 2^48 mod m
     uint32_t off28[12];  // smallest multiple of m that is >= 2^28 (makes signed accumulators non-negative)
+    uint32_t offtc[12];  // same, >= 2^25 (tensor-core digit recombination stays below 2^25 in magnitude)
     uint32_t u[12][4];   // CRT idempotents, 32-bit limbs (u_k < 2^118)
     uint32_t wlo[12], whi[12];  // w_k = round(2^48 u_k / M), split 32 + 16 bits
     uint32_t M[4];       // M limbs

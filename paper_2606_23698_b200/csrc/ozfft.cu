@@ -73,6 +73,7 @@ void fill_consts(DevConsts &c) {
         c.c32[k] = (uint32_t)((1ull << 32) % m);
         c.c48[k] = (uint32_t)((1ull << 48) % m);
         c.off28[k] = (uint32_t)((((1u << 28) + m - 1) / m) * m);
+        c.offtc[k] = (uint32_t)((((1u << 25) + m - 1) / m) * m);
         for (int l = 0; l < 4; l++) c.u[k][l] = (uint32_t)(C.u[k] >> (32 * l));
         c.wlo[k] = (uint32_t)C.w[k];
         c.whi[k] = (uint32_t)(C.w[k] >> 32);
@@ -152,30 +153,27 @@ bool add_axis(ozfft_plan_s *p, const AxisDesc &a, int axis, std::map<MatKey, std
     StageLaunch s1{}, s2{};
     s1.axis = s2.axis = axis;
     StageGeom &g1 = s1.g, &g2 = s2.g;
-    g1.K = q;
-    g1.nmat = 1;
-    g1.matsel = 0;
+    g1.K = q; g1.matsel = 0;
+    g2.K = pp; g2.matsel = 1; g2.ns = 32;
+    g1.ns = pp;
     if (!a.contiguous) {
         const long long I = a.inner;
-        g1.n0 = (int)(I / 32); g1.n1 = pp; g1.n2 = (int)a.outer;
-        g1.i0 = 32; g1.i1 = I; g1.i2 = a.N * I;
-        g1.lane = 1; g1.ji = pp * I; g1.ko = pp * I;
-        g2.K = pp; g2.n0 = (int)(I / 32); g2.n1 = 32; g2.n2 = (int)a.outer;
-        g2.i0 = 32; g2.i1 = pp * I; g2.i2 = a.N * I;
-        g2.o0 = 32; g2.o1 = I; g2.o2 = a.N * I;
-        g2.lane = 1; g2.ji = I; g2.ko = 32 * I; g2.matsel = 2;
+        g1.nb = g2.nb = (int)(I / 32); g1.no = g2.no = (int)a.outer;
+        g1.ib = 32; g1.is = I; g1.io = a.N * I;
+        g1.lane = 1; g1.ji = pp * I; g1.ko = pp * I; g1.order = 0;
+        g2.ib = 32; g2.is = pp * I; g2.io = a.N * I;
+        g2.ob = 32; g2.os = I; g2.oo = a.N * I;
+        g2.lane = 1; g2.ji = I; g2.ko = 32 * I; g2.order = 0;
     } else {
         const long long Pn = a.outer;
-        g1.n0 = pp; g1.n1 = (int)(Pn / 32); g1.n2 = 1;
-        g1.i0 = 1; g1.i1 = 32 * a.N; g1.i2 = 0;
-        g1.lane = a.N; g1.ji = pp; g1.ko = pp;
-        g2.K = pp; g2.n0 = 32; g2.n1 = (int)(Pn / 32); g2.n2 = 1;
-        g2.i0 = pp; g2.i1 = 32 * a.N; g2.i2 = 0;
-        g2.o0 = 1; g2.o1 = 32 * a.N; g2.o2 = 0;
-        g2.lane = a.N; g2.ji = 1; g2.ko = 32; g2.matsel = 1;
+        g1.nb = g2.nb = (int)(Pn / 32); g1.no = g2.no = 1;
+        g1.ib = 32 * a.N; g1.is = 1; g1.io = 0;
+        g1.lane = a.N; g1.ji = pp; g1.ko = pp; g1.order = 1;
+        g2.ib = 32 * a.N; g2.is = pp; g2.io = 0;
+        g2.ob = 32 * a.N; g2.os = 1; g2.oo = 0;
+        g2.lane = a.N; g2.ji = 1; g2.ko = 32; g2.order = 1;
     }
-    g1.o0 = g1.i0; g1.o1 = g1.i1; g1.o2 = g1.i2;
-    g2.nmat = 32;
+    g1.ob = g1.ib; g1.os = g1.is; g1.oo = g1.io;
     if (!get(q, 0, s1)) return false;
     p->stages.push_back(s1);
     if (two) {
@@ -187,8 +185,8 @@ bool add_axis(ozfft_plan_s *p, const AxisDesc &a, int axis, std::map<MatKey, std
 
 int pick_variant() {
     const char *v = getenv("OZFFT_VARIANT");
-    if (v && !strcmp(v, "tc")) return 1;
-    return 0;
+    if (v && !strcmp(v, "simt")) return 0;
+    return 1;
 }
 
 ozfft_plan_s *make_plan(int nx, int ny, int nz, int sign, bool batched1d) {
@@ -234,7 +232,7 @@ ozfft_plan_s *make_plan(int nx, int ny, int nz, int sign, bool batched1d) {
 bool valid(ozfft_plan p) { return p && p->magic == PLAN_MAGIC; }
 
 int launch_stage(ozfft_plan p, const StageLaunch &s, const void *src, void *dst, cudaStream_t st) {
-    const long long nt = tile_count(s.g);
+    const long long nt = (long long)s.g.nb * s.g.ns * s.g.no;
     if (p->variant == 1) return stage_tc_launch(s.g, src, dst, s.mat_tc, p->d_consts, st) ? OZFFT_OK : OZFFT_ECUDA;
     const size_t sm = (size_t)s.g.K * 32 * 16 + (size_t)12 * s.g.K * 32 * 4;
     static bool attr = false;

@@ -1,9 +1,10 @@
 // stage.cuh -- launch geometry shared by every stage kernel.
 //
 // One "stage" is one residue DFT-by-matrix over columns of length K (PAPER.md:115-124 Bailey six-step; Alg. 1
-// lines 1-7 for the first stage, 8-14 for the twiddle-fused second stage).  A tile is 32
-// columns that share one matrix.  Tile t decomposes as t = (t2*n1 + t1)*n0 + t0; all offsets are in complex
-// elements (16 bytes).
+// lines 1-7 for the first stage, 8-14 for the twiddle-fused second stage).  Columns come in
+// blocks of 32 (adjacent in memory where the axis allows).  A block has coordinates (b, s, o): b enumerates
+// blocks that share one matrix, s the matrix / sub-column index (j1 in stage 1, k2 in stage 2), o the outer
+// index.  All offsets are in complex elements (16 bytes).
 #pragma once
 #include <cstdint>
 
@@ -11,16 +12,20 @@ namespace oz {
 
 struct StageGeom {
     int K;               // contraction length = number of outputs per column (2..32)
-    int n0, n1, n2;      // tile grid
-    long long i0, i1, i2;  // input base strides per tile coordinate
-    long long o0, o1, o2;  // output base strides
-    long long lane;      // stride between the 32 columns of a tile (same for input and output)
+    int nb, ns, no;      // block grid
+    long long ib, is, io;  // input base strides per block coordinate
+    long long ob, os, oo;  // output base strides
+    long long lane;      // stride between the 32 columns of a block (same for input and output)
     long long ji;        // input stride between contraction elements j
     long long ko;        // output stride between output rows k
-    int matsel;          // matrix index of a tile: 0 -> 0, 1 -> t0, 2 -> t1
-    int nmat;
+    int matsel;          // matrix index of a block: 0 -> 0, 1 -> s
+    int order;           // enumeration order of a launch: 0 -> b fastest, 1 -> s fastest (then b), o slowest
 };
 
-__host__ __device__ inline long long tile_count(const StageGeom &g) { return (long long)g.n0 * g.n1 * g.n2; }
+// linear tile index -> (b, s, o) with nbt tiles along b
+__host__ __device__ inline void tile_coords(const StageGeom &g, long long t, int nbt, int &b, int &s, int &o) {
+    if (g.order == 0) { b = (int)(t % nbt); t /= nbt; s = (int)(t % g.ns); o = (int)(t / g.ns); }
+    else { s = (int)(t % g.ns); t /= g.ns; b = (int)(t % nbt); o = (int)(t / nbt); }
+}
 
 }  // namespace oz

@@ -29,14 +29,11 @@ __global__ void __launch_bounds__(SIMT_THREADS) stage_simt_kernel(StageGeom g, c
     if (tid < 32) { s_tmax[tid] = -100000; s_flag[tid] = 0; }
     __syncthreads();
 
-    long long t = blockIdx.x;
-    const int t0 = (int)(t % g.n0);
-    t /= g.n0;
-    const int t1 = (int)(t % g.n1);
-    const int t2 = (int)(t / g.n1);
-    const long long ibase = t0 * g.i0 + t1 * g.i1 + t2 * g.i2 + lane * g.lane;
-    const long long obase = t0 * g.o0 + t1 * g.o1 + t2 * g.o2 + lane * g.lane;
-    const int mid = g.matsel == 1 ? t0 : (g.matsel == 2 ? t1 : 0);
+    int tb, ts, to;
+    tile_coords(g, blockIdx.x, g.nb, tb, ts, to);
+    const long long ibase = tb * g.ib + ts * g.is + to * g.io + lane * g.lane;
+    const long long obase = tb * g.ob + ts * g.os + to * g.oo + lane * g.lane;
+    const int mid = g.matsel ? ts : 0;
 
     // ---- load + column exponent (a1, a2)
     for (int j = grp; j < K; j += SIMT_KG) {

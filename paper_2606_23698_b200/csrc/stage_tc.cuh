@@ -1,11 +1,272 @@
-// stage_tc.cuh -- tensor-core stage kernel (placeholder until the tcgen05 path lands).
+// stage_tc.cuh -- tensor-core stage kernel: one Bailey stage with the residue DFT on tcgen05 kind::i8 MMAs.
+//
+// Tile: 64 columns.  MMA row r (= TMEM lane r) = (column r/2, part r&1): the re row holds the digits of
+// [x_R ; -x_I], the im row those of [x_I ; x_R], so ONE matrix operand [a_R ; a_I] yields both parts
+// (direct 4-product complex form).
+// Digits (base 128, from canonical residues, PAPER.md:113 layout is the builder's): x = x0 + 128 x1,
+// a = a0 + 128 a1, a' = 128 a mod m = a'0 + 128 a'1, so  a x == (a0 x0 + a'0 x1) + 128 (a1 x0 + a'1 x1) (mod m):
+// two s32 accumulators per output and modulus, contraction over (half, j, digit) = 4 K bytes.
+// Per modulus i: deconstruct digits -> SMEM operand (double buffered) -> tcgen05.mma into TMEM (double
+// buffered) while the SIMT epilogue of modulus i-1 canonicalises its accumulators into the residue store;
+// matrix planes arrive by TMA bulk copy one modulus ahead.  After 12 moduli: exact CRT + lift + pack.
 #pragma once
 #include <vector>
+
 #include "arith.cuh"
 #include "stage.cuh"
 #include "tables.cuh"
+#include "tc.cuh"
+
 namespace oz {
-inline void build_mat_tc(std::vector<uint8_t> &h, int, int, int, const Twiddles &) { h.assign(16, 0); }
-inline bool stage_tc_prepare() { return false; }
-inline bool stage_tc_launch(const StageGeom &, const void *, void *, const uint8_t *, const DevConsts *, cudaStream_t) { return false; }
+
+constexpr int TC_THREADS = 512;
+constexpr int TC_TMEM_COLS = 128;
+
+// bytes of one modulus' matrix planes for padded length KP: rows n = 2k + d (d = digit 0/1), 4 KP bytes each,
+// stored in the canonical K-major no-swizzle core-matrix order [chunk = byte/16][row n][16 B]
+__host__ __device__ constexpr int tc_mat_bytes(int KP) { return 8 * KP * KP; }
+__host__ __device__ constexpr int tc_pad(int K) { return K < 8 ? 8 : K; }
+__host__ __device__ constexpr int tc_rs_stride(int KP) { return KP * 24 + 8; }
+__host__ __device__ constexpr size_t tc_smem_bytes(int KP) {
+    return 2 * (size_t)128 * 4 * KP + 2 * (size_t)tc_mat_bytes(KP) + (size_t)128 * tc_rs_stride(KP);
+}
+
+// host: digit planes of matrix set (K, fusedN) for all matrix ids and moduli: [mid][i][tc_mat_bytes]
+inline void build_mat_tc(std::vector<uint8_t> &h, int K, int fusedN, int sign, const Twiddles &T) {
+    const int KP = tc_pad(K), nmat = fusedN ? 32 : 1, MB = tc_mat_bytes(KP);
+    h.assign((size_t)nmat * 12 * MB, 0);
+    for (int mid = 0; mid < nmat; mid++)
+        for (int i = 0; i < 12; i++) {
+            uint8_t *dst = h.data() + ((size_t)mid * 12 + i) * MB;
+            const int m = kModuli[i];
+            for (int k = 0; k < K; k++)
+                for (int j = 0; j < K; j++) {
+                    const int t = fusedN ? (int)(((long)(TABLE_N / fusedN) * j * (mid + 32L * k)) % TABLE_N)
+                                         : (int)(((long)(TABLE_N / K) * j * k) % TABLE_N);
+                    const int a[2] = {residue_of(T.c[t], m), residue_of((int64_t)sign * T.s[t], m)};
+                    for (int half = 0; half < 2; half++) {
+                        const int av = a[half], ap = (av * 128) % m;  // a and a' = 128 a mod m
+                        for (int d = 0; d < 2; d++) {                 // digit plane -> output row 2k + d
+                            const int n = 2 * k + d;
+                            const int e0 = d ? av >> 7 : av & 127, e1 = d ? ap >> 7 : ap & 127;
+                            const int kap = half * 2 * KP + 2 * j;  // byte index in the contraction
+                            dst[(kap / 16) * (2 * KP * 16) + n * 16 + kap % 16] = (uint8_t)e0;
+                            dst[((kap + 1) / 16) * (2 * KP * 16) + n * 16 + (kap + 1) % 16] = (uint8_t)e1;
+                        }
+                    }
+                }
+        }
+}
+
+// -x per packed signed byte, no carries between bytes
+__device__ __forceinline__ uint32_t neg_bytes(uint32_t x) {
+    const uint32_t t = ~x;
+    return ((t & 0x7F7F7F7Fu) + 0x01010101u) ^ (t & 0x80808080u);
+}
+
+template <int KP>
+__global__ void __launch_bounds__(TC_THREADS, 1) stage_tc_kernel(StageGeom g, const uint64_t *__restrict__ in,
+                                                                 ulonglong2 *__restrict__ out,
+                                                                 const uint8_t *__restrict__ mat,
+                                                                 const DevConsts *__restrict__ cptr) {
+    constexpr int JC = KP / 4;         // contraction elements (and outputs) per thread
+    constexpr int ABYTES = 128 * 4 * KP;
+    constexpr int MB = tc_mat_bytes(KP);
+    constexpr int RS = tc_rs_stride(KP);
+    constexpr int NCOL = 2 * KP;       // accumulator columns per modulus
+    extern __shared__ __align__(128) uint8_t smem[];
+    __shared__ __align__(8) uint64_t bar_full[2], bar_load[2];
+    __shared__ uint32_t s_tmem;
+    __shared__ int s_tmax[64], s_flag[64];
+    __shared__ DevConsts c;
+    uint8_t *sA = smem, *sB = smem + 2 * ABYTES, *sR = smem + 2 * ABYTES + 2 * MB;
+
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+    const int row = (warp & 3) * 32 + lane, q = warp >> 2;
+    const int col = row >> 1, part = row & 1;
+    const int K = g.K;
+
+    for (int i = tid; i < (int)(sizeof(DevConsts) / 4); i += TC_THREADS) ((uint32_t *)&c)[i] = ((const uint32_t *)cptr)[i];
+    if (tid < 64) { s_tmax[tid] = -100000; s_flag[tid] = 0; }
+    if (warp == 0) tmem_alloc<TC_TMEM_COLS>(&s_tmem);
+    if (tid == 0) {
+        mbar_init(&bar_full[0], 1); mbar_init(&bar_full[1], 1);
+        mbar_init(&bar_load[0], 1); mbar_init(&bar_load[1], 1);
+        mbar_fence_init();
+    }
+    int tb, ts, to;
+    const int nbt = (g.nb + 1) >> 1;
+    tile_coords(g, blockIdx.x, nbt, tb, ts, to);
+    const int blk = 2 * tb + (col >> 5);
+    const bool colvalid = blk < g.nb;
+    const long long ibase = blk * g.ib + ts * g.is + to * g.io + (col & 31) * g.lane;
+    const long long obase = blk * g.ob + ts * g.os + to * g.oo + (col & 31) * g.lane;
+    const uint8_t *matbase = mat + (size_t)(g.matsel ? ts : 0) * 12 * MB;
+    tc_fence_before();
+    __syncthreads();
+    tc_fence_after();
+    const uint32_t tmem = s_tmem;
+    if (tid == 0) {  // matrix planes of moduli 0 and 1
+        mbar_expect_tx(&bar_load[0], MB);
+        bulk_g2s(sB, matbase, MB, &bar_load[0]);
+        mbar_expect_tx(&bar_load[1], MB);
+        bulk_g2s(sB + MB, matbase + MB, MB, &bar_load[1]);
+    }
+
+    // ---- a1/a2: load own part of own contraction elements, column exponent
+    uint64_t bits[JC];
+    {
+        int tm = -100000, fl = 0;
+#pragma unroll
+        for (int jj = 0; jj < JC; jj++) {
+            const int j = q * JC + jj;
+            bits[jj] = (colvalid && j < K) ? __ldg(in + 2 * (ibase + j * g.ji) + part) : 0ull;
+            int T;
+            const int cls = classify_top(bits[jj], T);
+            if (cls == CLS_FINITE) { fl |= 1; tm = max(tm, T); }
+            if (cls == CLS_NONFINITE) fl |= 2;
+        }
+        if (fl & 1) atomicMax(&s_tmax[col], tm);
+        if (fl) atomicOr(&s_flag[col], fl);
+    }
+    __syncthreads();
+    const int Tmax = s_tmax[col], flag = s_flag[col];
+    // ---- a3 (first half): quantise to 53-bit magnitudes, keep as 16-bit limbs
+    uint32_t xlo[JC], xhi[JC];
+    uint32_t negmask = 0;
+#pragma unroll
+    for (int jj = 0; jj < JC; jj++) {
+        const uint64_t a = (flag == 1) ? quantise_mag(bits[jj], Tmax) : 0ull;
+        xlo[jj] = (uint32_t)a;
+        xhi[jj] = (uint32_t)(a >> 32);
+        if (bits[jj] >> 63) negmask |= 1u << jj;
+    }
+
+    const uint32_t idesc = make_idesc(CFMT_S32, I8_S8, I8_S8, 128, NCOL);
+    const uint32_t lane_taddr = tmem + ((uint32_t)((warp & 3) * 32) << 16);
+
+    auto epilogue = [&](int i) {  // a5: recombine digits, canonicalise, park residues of modulus i
+        const int buf = i & 1;
+        mbar_wait(&bar_full[buf], (i >> 1) & 1);
+        tc_fence_after();
+        if (tid == 0 && i + 2 < 12) {  // MMA i is complete, so its matrix buffer can take modulus i+2
+            mbar_expect_tx(&bar_load[buf], MB);
+            bulk_g2s(sB + buf * MB, matbase + (size_t)(i + 2) * MB, MB, &bar_load[buf]);
+        }
+        uint32_t r[2 * JC];
+        const uint32_t ta = lane_taddr + buf * 64 + 2 * q * JC;
+        if constexpr (JC == 8) tmem_ld_x16(ta, r);
+        else if constexpr (JC == 4) tmem_ld_x8(ta, r);
+        else tmem_ld_x4(ta, r);
+        tmem_ld_wait();
+        const uint32_t m = c.m[i], mu = c.mu[i], off = c.offtc[i];
+#pragma unroll
+        for (int kk = 0; kk < JC; kk++) {
+            const uint32_t v = (uint32_t)((int)r[2 * kk] + 128 * (int)r[2 * kk + 1] + (int)off);
+            *(uint16_t *)(sR + row * RS + (q * JC + kk) * 24 + 2 * i) = (uint16_t)barrett(v, m, mu);
+        }
+        tc_fence_before();
+    };
+
+#pragma unroll 1
+    for (int i = 0; i < 12; i++) {
+        // ---- a3 (second half): residues mod m_i of own elements -> digit bytes (x0, x1) per element
+        const uint32_t m = c.m[i], mu = c.mu[i], c16 = c.c16[i], c32 = c.c32[i], c48 = c.c48[i];
+        uint32_t w[JC / 2];
+#pragma unroll
+        for (int jj = 0; jj < JC; jj++) {
+            uint32_t rr = (xlo[jj] & 0xFFFF) + (xlo[jj] >> 16) * c16 + (xhi[jj] & 0xFFFF) * c32 + (xhi[jj] >> 16) * c48;
+            rr = barrett(rr, m, mu);
+            if (((negmask >> jj) & 1) && rr) rr = m - rr;
+            const uint32_t hw = (rr & 0x7F) | ((rr << 1) & 0x1F00);
+            if (jj & 1) w[jj >> 1] |= hw << 16;
+            else w[jj >> 1] = hw;
+        }
+        // own digits go to the first half of the own row, the partner's (negated for the re row) to the second
+        uint8_t *A = sA + (i & 1) * ABYTES;
+#pragma unroll
+        for (int h = 0; h < 2; h++) {
+            uint32_t o[JC / 2];
+#pragma unroll
+            for (int t = 0; t < JC / 2; t++) {
+                const uint32_t pw = __shfl_xor_sync(0xFFFFFFFFu, w[t], 1);
+                o[t] = h == 0 ? w[t] : (part == 0 ? neg_bytes(pw) : pw);
+            }
+            const int kap = h * 2 * KP + q * JC * 2;  // first contraction byte this thread writes
+            uint8_t *dst = A + (kap >> 4) * (128 * 16) + row * 16 + (kap & 15);
+            if constexpr (JC == 8) *(uint4 *)dst = make_uint4(o[0], o[1], o[2], o[3]);
+            else if constexpr (JC == 4) *(uint2 *)dst = make_uint2(o[0], o[1]);
+            else *(uint32_t *)dst = o[0];
+        }
+        fence_async_smem();
+        tc_fence_before();
+        __syncthreads();
+        // ---- a4: residue DFT of modulus i on the tensor core
+        if (tid == 0) {
+            tc_fence_after();
+            mbar_wait(&bar_load[i & 1], (i >> 1) & 1);
+            const uint32_t a0 = smem_u32(A), b0 = smem_u32(sB + (i & 1) * MB);
+#pragma unroll
+            for (int ks = 0; ks < KP / 8; ks++) {
+                const uint64_t ad = make_sdesc(a0 + ks * 2 * 128 * 16, 128 * 16, 128);
+                const uint64_t bd = make_sdesc(b0 + ks * 2 * NCOL * 16, NCOL * 16, 128);
+                mma_i8_ss(tmem + (i & 1) * 64, ad, bd, idesc, ks > 0);
+            }
+            tc_commit(&bar_full[i & 1]);
+        }
+        if (i > 0) epilogue(i - 1);
+    }
+    epilogue(11);
+
+    // ---- a6-a9: exact CRT, lift, pack; a12: store (the re thread stores even k, the im thread odd k)
+    const int gexp = 53 + 52 - Tmax;
+#pragma unroll 1
+    for (int kk = 0; kk < JC; kk++) {
+        const int k = q * JC + kk;
+        uint64_t y;
+        if (flag & 2) y = 0x7FF8000000000000ull;
+        else if (flag == 0) y = 0;
+        else {
+            uint32_t v[12];
+            const uint2 *p = (const uint2 *)(sR + row * RS + k * 24);
+#pragma unroll
+            for (int t = 0; t < 3; t++) {
+                const uint2 u = p[t];
+                v[4 * t] = u.x & 0xFFFF; v[4 * t + 1] = u.x >> 16;
+                v[4 * t + 2] = u.y & 0xFFFF; v[4 * t + 3] = u.y >> 16;
+            }
+            y = pack_rne(crt_centre(v, c), gexp);
+        }
+        const uint32_t plo = __shfl_xor_sync(0xFFFFFFFFu, (uint32_t)y, 1), phi = __shfl_xor_sync(0xFFFFFFFFu, (uint32_t)(y >> 32), 1);
+        const uint64_t yp = ((uint64_t)phi << 32) | plo;
+        if (colvalid && k < K && (k & 1) == part) {
+            ulonglong2 o;
+            o.x = part ? yp : y;
+            o.y = part ? y : yp;
+            out[obase + k * g.ko] = o;
+        }
+    }
+    tc_fence_before();
+    __syncthreads();
+    if (warp == 0) tmem_dealloc<TC_TMEM_COLS>(tmem);
+}
+
+inline bool stage_tc_prepare() {
+    cudaError_t e = cudaFuncSetAttribute(stage_tc_kernel<32>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)tc_smem_bytes(32));
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(stage_tc_kernel<16>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)tc_smem_bytes(16));
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(stage_tc_kernel<8>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)tc_smem_bytes(8));
+    return e == cudaSuccess;
+}
+
+inline bool stage_tc_launch(const StageGeom &g, const void *src, void *dst, const uint8_t *mat, const DevConsts *dc, cudaStream_t st) {
+    const int KP = tc_pad(g.K);
+    const long long nt = (long long)((g.nb + 1) / 2) * g.ns * g.no;
+    const uint64_t *in = (const uint64_t *)src;
+    ulonglong2 *out = (ulonglong2 *)dst;
+    if (KP == 32) stage_tc_kernel<32><<<(unsigned)nt, TC_THREADS, tc_smem_bytes(32), st>>>(g, in, out, mat, dc);
+    else if (KP == 16) stage_tc_kernel<16><<<(unsigned)nt, TC_THREADS, tc_smem_bytes(16), st>>>(g, in, out, mat, dc);
+    else stage_tc_kernel<8><<<(unsigned)nt, TC_THREADS, tc_smem_bytes(8), st>>>(g, in, out, mat, dc);
+    return cudaGetLastError() == cudaSuccess;
+}
+
 }  // namespace oz

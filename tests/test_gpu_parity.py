@@ -8,6 +8,13 @@ pytestmark = pytest.mark.gpu
 TOL_F128 = 5e-15  # north_star: normwise relative error vs the __float128 naive DFT
 
 
+@pytest.fixture(autouse=True, params=["tc", "simt"])
+def variant(request, monkeypatch):
+    """every parity case runs on the tensor-core kernel and on the all-SIMT cross-check kernel"""
+    monkeypatch.setenv("OZFFT_VARIANT", request.param)
+    return request.param
+
+
 def _torch():
     import torch
     assert torch.cuda.is_available()
