@@ -21,7 +21,14 @@ struct DevConsts {
     uint32_t wlo[12], whi[12];  // w_k = round(2^48 u_k / M), split 32 + 16 bits
     uint32_t M[4];       // M limbs
     uint32_t Mh[4];      // M/2 limbs
+    uint32_t c18[12];    // 2^18 mod m
+    uint32_t c36[12];    // 2^36 mod m
+    uint32_t m2[12];     // 2 m
+    uint32_t zC;         // round(2^149 / M): zhat = (umulhi(E >> 104, zC) + 2^12) >> 13
 };
+
+// the same constants in the constant bank (uniform operands, no shared-memory loads); set by stage_tc_prepare
+__constant__ DevConsts kc;
 
 // value class of an fp64 bit pattern; T = floor(log2 |x|) for finite nonzero x
 enum { CLS_ZERO = 0, CLS_FINITE = 1, CLS_NONFINITE = 2 };
@@ -128,6 +135,85 @@ __device__ __forceinline__ i128 crt_centre(const uint32_t *v, const DevConsts &c
     if (R >= Mh) R -= (i128)M;
     if (R < -Mh) R += (i128)M;
     return R;
+}
+
+// ---------------------------------------------------------------------------------------------------
+// 32-bit limb forms used by the tensor-core kernel (same integers as crt_centre / pack_rne above).
+
+// r = a - b over four 32-bit limbs (mod 2^128), one borrow chain
+__device__ __forceinline__ void sub128(uint32_t *r, uint32_t a0, uint32_t a1, uint32_t a2, uint32_t a3, uint32_t b0,
+                                       uint32_t b1, uint32_t b2, uint32_t b3) {
+    asm("sub.cc.u32 %0, %4, %8;\n\tsubc.cc.u32 %1, %5, %9;\n\tsubc.cc.u32 %2, %6, %10;\n\tsubc.u32 %3, %7, %11;"
+        : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3])
+        : "r"(a0), "r"(a1), "r"(a2), "r"(a3), "r"(b0), "r"(b1), "r"(b2), "r"(b3));
+}
+// |x| of a two's-complement 128-bit value: (x ^ sm) + (sm & 1) with sm = sign mask, one carry chain
+__device__ __forceinline__ void abs128(uint32_t *a, const uint32_t *x, uint32_t sm) {
+    asm("add.cc.u32 %0, %4, %8;\n\taddc.cc.u32 %1, %5, 0;\n\taddc.cc.u32 %2, %6, 0;\n\taddc.u32 %3, %7, 0;"
+        : "=r"(a[0]), "=r"(a[1]), "=r"(a[2]), "=r"(a[3])
+        : "r"(x[0] ^ sm), "r"(x[1] ^ sm), "r"(x[2] ^ sm), "r"(x[3] ^ sm), "r"(sm & 1));
+}
+
+// Direct CRT E = sum_k v_k u_k (Eq. 17) on residues that need not be canonical (v_k < 2^13, any
+// representative: m_k u_k == 0 mod M), quotient zhat = round(E/M) read off the top 30 bits of E (the lift of
+// PAPER.md:370 with the fraction taken from E itself), R = E - zhat M, two-sided centring.
+// r[0..3]: two's-complement limbs of R in [-M/2, M/2).
+__device__ __forceinline__ void crt_limbs(const uint32_t *v, uint32_t *r) {
+    uint64_t a0 = 0, a1 = 0, a2 = 0, a3 = 0;
+#pragma unroll
+    for (int k = 0; k < 12; k++) {
+        a0 += (uint64_t)v[k] * kc.u[k][0];
+        a1 += (uint64_t)v[k] * kc.u[k][1];
+        a2 += (uint64_t)v[k] * kc.u[k][2];
+        a3 += (uint64_t)v[k] * kc.u[k][3];
+    }
+    a1 += a0 >> 32;
+    a2 += a1 >> 32;
+    a3 += a2 >> 32;
+    const uint32_t e0 = (uint32_t)a0, e1 = (uint32_t)a1, e2 = (uint32_t)a2, e3 = (uint32_t)a3, e4 = (uint32_t)(a3 >> 32);
+    const uint32_t T = __funnelshift_r(e3, e4, 8);  // E >> 104
+    const uint32_t z = (__umulhi(T, kc.zC) + (1u << 12)) >> 13;
+    uint64_t p0 = (uint64_t)z * kc.M[0];
+    uint64_t p1 = (uint64_t)z * kc.M[1] + (p0 >> 32);
+    uint64_t p2 = (uint64_t)z * kc.M[2] + (p1 >> 32);
+    uint64_t p3 = (uint64_t)z * kc.M[3] + (p2 >> 32);
+    sub128(r, e0, e1, e2, e3, (uint32_t)p0, (uint32_t)p1, (uint32_t)p2, (uint32_t)p3);
+    // |R| can reach M/2 only if the top limb does; everything else skips the exact comparison
+    if ((uint32_t)(r[3] + kc.Mh[3]) >= 2 * kc.Mh[3]) {
+        const u128 M = ((u128)kc.M[3] << 96) | ((u128)kc.M[2] << 64) | ((u128)kc.M[1] << 32) | kc.M[0];
+        i128 R = (i128)(((u128)r[3] << 96) | ((u128)r[2] << 64) | ((u128)r[1] << 32) | r[0]);
+        const i128 Mh = (i128)(M >> 1);
+        if (R >= Mh) R -= (i128)M;
+        if (R < -Mh) R += (i128)M;
+        r[0] = (uint32_t)R; r[1] = (uint32_t)((u128)R >> 32); r[2] = (uint32_t)((u128)R >> 64); r[3] = (uint32_t)((u128)R >> 96);
+    }
+}
+
+// RNE_fp64(R * 2^-g) from two's-complement limbs (DESIGN.md A.6); normal-range results take the limb path,
+// zero / subnormal / overflowing ones the generic pack_rne.
+__device__ __forceinline__ uint64_t pack_limbs(const uint32_t *r, int g) {
+    const uint32_t sm = (uint32_t)((int32_t)r[3] >> 31);  // all ones if negative
+    uint32_t av[4];
+    abs128(av, r, sm);
+    uint32_t a0 = av[0], a1 = av[1], a2 = av[2], a3 = av[3];
+    const uint64_t hi = ((uint64_t)a3 << 32) | a2, lo = ((uint64_t)a1 << 32) | a0;
+    const int s = hi ? __clzll((long long)hi) : 64 + __clzll((long long)lo);  // left shift that puts the top bit at 127
+    const int X = 127 - s - g;
+    if (X < -1022 || X > 1023 || s >= 128) {
+        const i128 R = (i128)(((u128)r[3] << 96) | ((u128)r[2] << 64) | ((u128)r[1] << 32) | r[0]);
+        return pack_rne(R, g);
+    }
+    if (s & 64) { a3 = a1; a2 = a0; a1 = 0; a0 = 0; }
+    if (s & 32) { a3 = a2; a2 = a1; a1 = a0; a0 = 0; }
+    const int bs = s & 31;
+    const uint32_t m3 = __funnelshift_l(a2, a3, bs), m2 = __funnelshift_l(a1, a2, bs), m1 = __funnelshift_l(a0, a1, bs), m0 = a0 << bs;
+    // top 53 bits = m3 : m2[31:11]; round bit m2[10]; sticky = rest
+    const uint32_t qhi = m3 >> 11, qlo = __funnelshift_r(m2, m3, 11);
+    const uint32_t sticky = ((m2 & 0x3FF) | m1 | m0) != 0;
+    const uint32_t inc = (m2 >> 10) & (sticky | qlo) & 1;
+    // exponent field X+1023 enters as (X+1022) << 52 plus the hidden bit; a mantissa carry bumps it by itself
+    uint64_t bits = ((uint64_t)(uint32_t)(X + 1022) << 52) + (((uint64_t)qhi << 32) | qlo) + inc;
+    return bits | ((uint64_t)(sm & 0x80000000u) << 32);
 }
 
 }  // namespace oz

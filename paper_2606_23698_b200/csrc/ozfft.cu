@@ -78,6 +78,23 @@ void fill_consts(DevConsts &c) {
         c.wlo[k] = (uint32_t)C.w[k];
         c.whi[k] = (uint32_t)(C.w[k] >> 32);
     }
+    for (int k = 0; k < R_MOD; k++) {
+        const uint32_t m = (uint32_t)kModuli[k];
+        c.c18[k] = (uint32_t)((1ull << 18) % m);
+        c.c36[k] = (uint32_t)((1ull << 36) % m);
+        c.m2[k] = 2 * m;
+    }
+    {  // zC = round(2^149 / M) by binary long division
+        u128 rem = 1;
+        uint64_t q = 0;
+        for (int b = 0; b < 149; b++) {
+            rem <<= 1;
+            q <<= 1;
+            if (rem >= C.M) { rem -= C.M; q |= 1; }
+        }
+        if (rem * 2 >= C.M) q++;
+        c.zC = (uint32_t)q;
+    }
     for (int l = 0; l < 4; l++) {
         c.M[l] = (uint32_t)(C.M >> (32 * l));
         c.Mh[l] = (uint32_t)(C.Mhalf >> (32 * l));
@@ -219,7 +236,7 @@ ozfft_plan_s *make_plan(int nx, int ny, int nz, int sign, bool batched1d) {
         ok = cuda_ok(cudaMalloc(&p->work, (size_t)p->count * 16), "cudaMalloc(workspace)");
         if (ok) p->dev_bytes += (size_t)p->count * 16;
     }
-    if (ok && p->variant == 1) ok = stage_tc_prepare();
+    if (ok && p->variant == 1) ok = stage_tc_prepare(hc);
     if (!ok) {
         std::string keep = g_err;
         ozfft_plan_destroy(p);

@@ -58,11 +58,8 @@ inline void build_mat_tc(std::vector<uint8_t> &h, int K, int fusedN, int sign, c
         }
 }
 
-// -x per packed signed byte, no carries between bytes
-__device__ __forceinline__ uint32_t neg_bytes(uint32_t x) {
-    const uint32_t t = ~x;
-    return ((t & 0x7F7F7F7Fu) + 0x01010101u) ^ (t & 0x80808080u);
-}
+// -x per packed byte for bytes in [0, 127] (digits are non-negative), no carries between bytes
+__device__ __forceinline__ uint32_t neg_bytes(uint32_t x) { return ((x ^ 0x7F7F7F7Fu) + 0x01010101u) ^ 0x80808080u; }
 
 template <int KP>
 __global__ void __launch_bounds__(TC_THREADS, 1) stage_tc_kernel(StageGeom g, const uint64_t *__restrict__ in,
@@ -78,7 +75,6 @@ __global__ void __launch_bounds__(TC_THREADS, 1) stage_tc_kernel(StageGeom g, co
     __shared__ __align__(8) uint64_t bar_full[2], bar_load[2];
     __shared__ uint32_t s_tmem;
     __shared__ int s_tmax[64], s_flag[64];
-    __shared__ DevConsts c;
     uint8_t *sA = smem, *sB = smem + 2 * ABYTES, *sR = smem + 2 * ABYTES + 2 * MB;
 
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
@@ -86,7 +82,6 @@ __global__ void __launch_bounds__(TC_THREADS, 1) stage_tc_kernel(StageGeom g, co
     const int col = row >> 1, part = row & 1;
     const int K = g.K;
 
-    for (int i = tid; i < (int)(sizeof(DevConsts) / 4); i += TC_THREADS) ((uint32_t *)&c)[i] = ((const uint32_t *)cptr)[i];
     if (tid < 64) { s_tmax[tid] = -100000; s_flag[tid] = 0; }
     if (warp == 0) tmem_alloc<TC_TMEM_COLS>(&s_tmem);
     if (tid == 0) {
@@ -131,14 +126,15 @@ __global__ void __launch_bounds__(TC_THREADS, 1) stage_tc_kernel(StageGeom g, co
     }
     __syncthreads();
     const int Tmax = s_tmax[col], flag = s_flag[col];
-    // ---- a3 (first half): quantise to 53-bit magnitudes, keep as 16-bit limbs
-    uint32_t xlo[JC], xhi[JC];
+    // ---- a3 (first half): quantise to 53-bit magnitudes, keep as 18/18/17-bit limbs (PAPER.md:190 planes)
+    uint32_t x0[JC], x1[JC], x2[JC];
     uint32_t negmask = 0;
 #pragma unroll
     for (int jj = 0; jj < JC; jj++) {
         const uint64_t a = (flag == 1) ? quantise_mag(bits[jj], Tmax) : 0ull;
-        xlo[jj] = (uint32_t)a;
-        xhi[jj] = (uint32_t)(a >> 32);
+        x0[jj] = (uint32_t)a & 0x3FFFF;
+        x1[jj] = (uint32_t)(a >> 18) & 0x3FFFF;
+        x2[jj] = (uint32_t)(a >> 36);
         if (bits[jj] >> 63) negmask |= 1u << jj;
     }
 
@@ -159,11 +155,11 @@ __global__ void __launch_bounds__(TC_THREADS, 1) stage_tc_kernel(StageGeom g, co
         else if constexpr (JC == 4) tmem_ld_x8(ta, r);
         else tmem_ld_x4(ta, r);
         tmem_ld_wait();
-        const uint32_t m = c.m[i], mu = c.mu[i], off = c.offtc[i];
+        const uint32_t m = kc.m[i], mu = kc.mu[i], off = kc.offtc[i];
 #pragma unroll
-        for (int kk = 0; kk < JC; kk++) {
-            const uint32_t v = (uint32_t)((int)r[2 * kk] + 128 * (int)r[2 * kk + 1] + (int)off);
-            *(uint16_t *)(sR + row * RS + (q * JC + kk) * 24 + 2 * i) = (uint16_t)barrett(v, m, mu);
+        for (int kk = 0; kk < JC; kk++) {  // residue left in [0, 2m): any representative serves the CRT
+            const uint32_t v = (uint32_t)((int)r[2 * kk + 1] * 128 + (int)r[2 * kk]) + off;
+            *(uint16_t *)(sR + row * RS + (q * JC + kk) * 24 + 2 * i) = (uint16_t)(v - __umulhi(v, mu) * m);
         }
         tc_fence_before();
     };
@@ -171,14 +167,14 @@ __global__ void __launch_bounds__(TC_THREADS, 1) stage_tc_kernel(StageGeom g, co
 #pragma unroll 1
     for (int i = 0; i < 12; i++) {
         // ---- a3 (second half): residues mod m_i of own elements -> digit bytes (x0, x1) per element
-        const uint32_t m = c.m[i], mu = c.mu[i], c16 = c.c16[i], c32 = c.c32[i], c48 = c.c48[i];
+        const uint32_t mu = kc.mu[i], m = kc.m[i], m2 = kc.m2[i], c18 = kc.c18[i], c36 = kc.c36[i];
         uint32_t w[JC / 2];
 #pragma unroll
         for (int jj = 0; jj < JC; jj++) {
-            uint32_t rr = (xlo[jj] & 0xFFFF) + (xlo[jj] >> 16) * c16 + (xhi[jj] & 0xFFFF) * c32 + (xhi[jj] >> 16) * c48;
-            rr = barrett(rr, m, mu);
-            if (((negmask >> jj) & 1) && rr) rr = m - rr;
-            const uint32_t hw = (rr & 0x7F) | ((rr << 1) & 0x1F00);
+            uint32_t rr = x0[jj] + x1[jj] * c18 + x2[jj] * c36;  // < 2^30
+            rr -= __umulhi(rr, mu) * m;                           // in [0, 2m)
+            if ((negmask >> jj) & 1) rr = m2 - rr;                // -x: in (0, 2m]
+            const uint32_t hw = rr + (rr & 0xFF80u);              // digits x0 = rr & 127, x1 = rr >> 7 as two bytes
             if (jj & 1) w[jj >> 1] |= hw << 16;
             else w[jj >> 1] = hw;
         }
@@ -235,7 +231,9 @@ __global__ void __launch_bounds__(TC_THREADS, 1) stage_tc_kernel(StageGeom g, co
                 v[4 * t] = u.x & 0xFFFF; v[4 * t + 1] = u.x >> 16;
                 v[4 * t + 2] = u.y & 0xFFFF; v[4 * t + 3] = u.y >> 16;
             }
-            y = pack_rne(crt_centre(v, c), gexp);
+            uint32_t R[4];
+            crt_limbs(v, R);
+            y = pack_limbs(R, gexp);
         }
         const uint32_t plo = __shfl_xor_sync(0xFFFFFFFFu, (uint32_t)y, 1), phi = __shfl_xor_sync(0xFFFFFFFFu, (uint32_t)(y >> 32), 1);
         const uint64_t yp = ((uint64_t)phi << 32) | plo;
@@ -251,8 +249,9 @@ __global__ void __launch_bounds__(TC_THREADS, 1) stage_tc_kernel(StageGeom g, co
     if (warp == 0) tmem_dealloc<TC_TMEM_COLS>(tmem);
 }
 
-inline bool stage_tc_prepare() {
-    cudaError_t e = cudaFuncSetAttribute(stage_tc_kernel<32>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)tc_smem_bytes(32));
+inline bool stage_tc_prepare(const DevConsts &hc) {
+    cudaError_t e = cudaMemcpyToSymbol(kc, &hc, sizeof(DevConsts));
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(stage_tc_kernel<32>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)tc_smem_bytes(32));
     if (e == cudaSuccess) e = cudaFuncSetAttribute(stage_tc_kernel<16>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)tc_smem_bytes(16));
     if (e == cudaSuccess) e = cudaFuncSetAttribute(stage_tc_kernel<8>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)tc_smem_bytes(8));
     return e == cudaSuccess;
