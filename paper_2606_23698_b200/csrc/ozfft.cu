@@ -186,6 +186,9 @@ bool add_axis(ozfft_plan_s *p, const AxisDesc &a, int axis, std::map<MatKey, std
         g1.nb = g2.nb = (int)(Pn / 32); g1.no = g2.no = 1;
         g1.ib = 32 * a.N; g1.is = 1; g1.io = 0;
         g1.lane = a.N; g1.ji = pp; g1.ko = pp; g1.order = 1;
+        if (two && pp == 32) {  // N = 1024: a block is one pencil, lanes along j1 (adjacent elements): coalesced
+            g1.nb = (int)Pn; g1.ns = 1; g1.ib = a.N; g1.is = 0; g1.lane = 1; g1.order = 0;
+        }
         g2.ib = 32 * a.N; g2.is = pp; g2.io = 0;
         g2.ob = 32 * a.N; g2.os = 1; g2.oo = 0;
         g2.lane = a.N; g2.ji = 1; g2.ko = 32; g2.order = 1;

@@ -19,7 +19,8 @@
 
 namespace oz {
 
-constexpr int TC_THREADS = 512;
+// threads per CTA = 128 * Q: Q thread groups share each MMA row and split its contraction elements / outputs
+__host__ __device__ constexpr int tc_q(int) { return 4; }
 constexpr int TC_TMEM_COLS = 128;
 
 // bytes of one modulus' matrix planes for padded length KP: rows n = 2k + d (d = digit 0/1), 4 KP bytes each,
@@ -62,11 +63,11 @@ inline void build_mat_tc(std::vector<uint8_t> &h, int K, int fusedN, int sign, c
 __device__ __forceinline__ uint32_t neg_bytes(uint32_t x) { return ((x ^ 0x7F7F7F7Fu) + 0x01010101u) ^ 0x80808080u; }
 
 template <int KP>
-__global__ void __launch_bounds__(TC_THREADS, 1) stage_tc_kernel(StageGeom g, const uint64_t *__restrict__ in,
+__global__ void __launch_bounds__(128 * tc_q(KP), KP >= 32 ? 1 : 2) stage_tc_kernel(StageGeom g, const uint64_t *__restrict__ in,
                                                                  ulonglong2 *__restrict__ out,
-                                                                 const uint8_t *__restrict__ mat,
-                                                                 const DevConsts *__restrict__ cptr) {
-    constexpr int JC = KP / 4;         // contraction elements (and outputs) per thread
+                                                                 const uint8_t *__restrict__ mat, long long ntiles) {
+    constexpr int Q = tc_q(KP);
+    constexpr int JC = KP / Q;         // contraction elements (and outputs) per thread
     constexpr int ABYTES = 128 * 4 * KP;
     constexpr int MB = tc_mat_bytes(KP);
     constexpr int RS = tc_rs_stride(KP);
@@ -74,58 +75,84 @@ __global__ void __launch_bounds__(TC_THREADS, 1) stage_tc_kernel(StageGeom g, co
     extern __shared__ __align__(128) uint8_t smem[];
     __shared__ __align__(8) uint64_t bar_full[2], bar_load[2];
     __shared__ uint32_t s_tmem;
-    __shared__ int s_tmax[64], s_flag[64];
+    __shared__ int s_tmax[2][64], s_flag[2][64];
     uint8_t *sA = smem, *sB = smem + 2 * ABYTES, *sR = smem + 2 * ABYTES + 2 * MB;
 
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
-    const int row = (warp & 3) * 32 + lane, q = warp >> 2;
+    const int row = (warp & 3) * 32 + lane, q = warp >> 2;  // q < Q
     const int col = row >> 1, part = row & 1;
     const int K = g.K;
+    const int nbt = (g.nb + 1) >> 1;
 
-    if (tid < 64) { s_tmax[tid] = -100000; s_flag[tid] = 0; }
+    if (tid < 64) { s_tmax[0][tid] = s_tmax[1][tid] = -100000; s_flag[0][tid] = s_flag[1][tid] = 0; }
     if (warp == 0) tmem_alloc<TC_TMEM_COLS>(&s_tmem);
     if (tid == 0) {
         mbar_init(&bar_full[0], 1); mbar_init(&bar_full[1], 1);
         mbar_init(&bar_load[0], 1); mbar_init(&bar_load[1], 1);
         mbar_fence_init();
     }
-    int tb, ts, to;
-    const int nbt = (g.nb + 1) >> 1;
-    tile_coords(g, blockIdx.x, nbt, tb, ts, to);
-    const int blk = 2 * tb + (col >> 5);
-    const bool colvalid = blk < g.nb;
-    const long long ibase = blk * g.ib + ts * g.is + to * g.io + (col & 31) * g.lane;
-    const long long obase = blk * g.ob + ts * g.os + to * g.oo + (col & 31) * g.lane;
-    const uint8_t *matbase = mat + (size_t)(g.matsel ? ts : 0) * 12 * MB;
     tc_fence_before();
     __syncthreads();
     tc_fence_after();
     const uint32_t tmem = s_tmem;
-    if (tid == 0) {  // matrix planes of moduli 0 and 1
+    const uint32_t idesc = make_idesc(CFMT_S32, I8_S8, I8_S8, 128, NCOL);
+    const uint32_t lane_taddr = tmem + ((uint32_t)((warp & 3) * 32) << 16);
+
+    // per-tile addressing: (valid, input base, output base, matrix base)
+    auto locate = [&](long long t, bool &valid, long long &ib, long long &ob, const uint8_t *&mb) {
+        int tb, ts, to;
+        tile_coords(g, t, nbt, tb, ts, to);
+        const int blk = 2 * tb + (col >> 5);
+        valid = blk < g.nb;
+        ib = blk * g.ib + ts * g.is + to * g.io + (col & 31) * g.lane;
+        ob = blk * g.ob + ts * g.os + to * g.oo + (col & 31) * g.lane;
+        mb = mat + (size_t)(g.matsel ? ts : 0) * 12 * MB;
+    };
+    auto load_inputs = [&](bool valid, long long ib, uint64_t *bits) {  // a1: own part of own contraction elements
+#pragma unroll
+        for (int jj = 0; jj < JC; jj++) {
+            const int j = q * JC + jj;
+            bits[jj] = (valid && j < K) ? __ldg(in + 2 * (ib + j * g.ji) + part) : 0ull;
+        }
+    };
+
+    long long tile = blockIdx.x;
+    if (tile >= ntiles) {  // (never with grid <= ntiles) still release TMEM
+        if (warp == 0) tmem_dealloc<TC_TMEM_COLS>(tmem);
+        return;
+    }
+    bool colvalid;
+    long long ibase, obase;
+    const uint8_t *matbase;
+    locate(tile, colvalid, ibase, obase, matbase);
+    if (tid == 0) {  // matrix planes of moduli 0 and 1 of the first tile
         mbar_expect_tx(&bar_load[0], MB);
         bulk_g2s(sB, matbase, MB, &bar_load[0]);
         mbar_expect_tx(&bar_load[1], MB);
         bulk_g2s(sB + MB, matbase + MB, MB, &bar_load[1]);
     }
-
-    // ---- a1/a2: load own part of own contraction elements, column exponent
     uint64_t bits[JC];
+    load_inputs(colvalid, ibase, bits);
+    int tpar = 0;
+
+#pragma unroll 1
+    for (; tile < ntiles; tile += gridDim.x, tpar ^= 1) {
+    // ---- a2: column exponent
     {
         int tm = -100000, fl = 0;
 #pragma unroll
         for (int jj = 0; jj < JC; jj++) {
-            const int j = q * JC + jj;
-            bits[jj] = (colvalid && j < K) ? __ldg(in + 2 * (ibase + j * g.ji) + part) : 0ull;
             int T;
             const int cls = classify_top(bits[jj], T);
             if (cls == CLS_FINITE) { fl |= 1; tm = max(tm, T); }
             if (cls == CLS_NONFINITE) fl |= 2;
         }
-        if (fl & 1) atomicMax(&s_tmax[col], tm);
-        if (fl) atomicOr(&s_flag[col], fl);
+        if (fl & 1) atomicMax(&s_tmax[tpar][col], tm);
+        if (fl) atomicOr(&s_flag[tpar][col], fl);
     }
     __syncthreads();
-    const int Tmax = s_tmax[col], flag = s_flag[col];
+    const int Tmax = s_tmax[tpar][col], flag = s_flag[tpar][col];
+    if (tid < 64) { s_tmax[tpar ^ 1][tid] = -100000; s_flag[tpar ^ 1][tid] = 0; }  // for the next tile
     // ---- a3 (first half): quantise to 53-bit magnitudes, keep as 18/18/17-bit limbs (PAPER.md:190 planes)
     uint32_t x0[JC], x1[JC], x2[JC];
     uint32_t negmask = 0;
@@ -137,17 +164,23 @@ __global__ void __launch_bounds__(TC_THREADS, 1) stage_tc_kernel(StageGeom g, co
         x2[jj] = (uint32_t)(a >> 36);
         if (bits[jj] >> 63) negmask |= 1u << jj;
     }
-
-    const uint32_t idesc = make_idesc(CFMT_S32, I8_S8, I8_S8, 128, NCOL);
-    const uint32_t lane_taddr = tmem + ((uint32_t)((warp & 3) * 32) << 16);
+    // ---- prefetch the next tile's inputs; they are consumed at the top of the next iteration
+    const long long ntile = tile + gridDim.x;
+    const bool more = ntile < ntiles;
+    bool nvalid = false;
+    long long nib = 0, nob = 0;
+    const uint8_t *nmat = matbase;
+    if (more) locate(ntile, nvalid, nib, nob, nmat);
+    load_inputs(more && nvalid, nib, bits);
 
     auto epilogue = [&](int i) {  // a5: recombine digits, canonicalise, park residues of modulus i
         const int buf = i & 1;
         mbar_wait(&bar_full[buf], (i >> 1) & 1);
         tc_fence_after();
-        if (tid == 0 && i + 2 < 12) {  // MMA i is complete, so its matrix buffer can take modulus i+2
+        if (tid == 0 && (i + 2 < 12 || more)) {  // MMA i is complete: its matrix buffer takes modulus i+2 (or the
+            const uint8_t *src = i + 2 < 12 ? matbase + (size_t)(i + 2) * MB : nmat + (size_t)(i - 10) * MB;  // next tile's)
             mbar_expect_tx(&bar_load[buf], MB);
-            bulk_g2s(sB + buf * MB, matbase + (size_t)(i + 2) * MB, MB, &bar_load[buf]);
+            bulk_g2s(sB + buf * MB, src, MB, &bar_load[buf]);
         }
         uint32_t r[2 * JC];
         const uint32_t ta = lane_taddr + buf * 64 + 2 * q * JC;
@@ -155,11 +188,11 @@ __global__ void __launch_bounds__(TC_THREADS, 1) stage_tc_kernel(StageGeom g, co
         else if constexpr (JC == 4) tmem_ld_x8(ta, r);
         else tmem_ld_x4(ta, r);
         tmem_ld_wait();
-        const uint32_t m = kc.m[i], mu = kc.mu[i], off = kc.offtc[i];
+        const uint32_t negm = 0u - kc.m[i], mu = kc.mu[i], off = kc.offtc[i];
 #pragma unroll
         for (int kk = 0; kk < JC; kk++) {  // residue left in [0, 2m): any representative serves the CRT
             const uint32_t v = (uint32_t)((int)r[2 * kk + 1] * 128 + (int)r[2 * kk]) + off;
-            *(uint16_t *)(sR + row * RS + (q * JC + kk) * 24 + 2 * i) = (uint16_t)(v - __umulhi(v, mu) * m);
+            *(uint16_t *)(sR + row * RS + (q * JC + kk) * 24 + 2 * i) = (uint16_t)(v + __umulhi(v, mu) * negm);
         }
         tc_fence_before();
     };
@@ -167,12 +200,12 @@ __global__ void __launch_bounds__(TC_THREADS, 1) stage_tc_kernel(StageGeom g, co
 #pragma unroll 1
     for (int i = 0; i < 12; i++) {
         // ---- a3 (second half): residues mod m_i of own elements -> digit bytes (x0, x1) per element
-        const uint32_t mu = kc.mu[i], m = kc.m[i], m2 = kc.m2[i], c18 = kc.c18[i], c36 = kc.c36[i];
+        const uint32_t mu = kc.mu[i], negm = 0u - kc.m[i], m2 = kc.m2[i], c18 = kc.c18[i], c36 = kc.c36[i];
         uint32_t w[JC / 2];
 #pragma unroll
         for (int jj = 0; jj < JC; jj++) {
             uint32_t rr = x0[jj] + x1[jj] * c18 + x2[jj] * c36;  // < 2^30
-            rr -= __umulhi(rr, mu) * m;                           // in [0, 2m)
+            rr += __umulhi(rr, mu) * negm;                        // in [0, 2m)
             if ((negmask >> jj) & 1) rr = m2 - rr;                // -x: in (0, 2m]
             const uint32_t hw = rr + (rr & 0xFF80u);              // digits x0 = rr & 127, x1 = rr >> 7 as two bytes
             if (jj & 1) w[jj >> 1] |= hw << 16;
@@ -244,6 +277,8 @@ __global__ void __launch_bounds__(TC_THREADS, 1) stage_tc_kernel(StageGeom g, co
             out[obase + k * g.ko] = o;
         }
     }
+    colvalid = nvalid; ibase = nib; obase = nob; matbase = nmat;
+    }  // tile loop
     tc_fence_before();
     __syncthreads();
     if (warp == 0) tmem_dealloc<TC_TMEM_COLS>(tmem);
@@ -257,15 +292,44 @@ inline bool stage_tc_prepare(const DevConsts &hc) {
     return e == cudaSuccess;
 }
 
-inline bool stage_tc_launch(const StageGeom &g, const void *src, void *dst, const uint8_t *mat, const DevConsts *dc, cudaStream_t st) {
+template <int KP>
+inline bool stage_tc_launch_kp(const StageGeom &g, const uint64_t *in, ulonglong2 *out, const uint8_t *mat, long long nt, int sms, cudaStream_t st) {
+    static int per_sm = 0;  // resident CTAs per SM for this instantiation (persistent grid = sms * per_sm)
+    if (!per_sm) {
+        cudaFuncAttributes fa;
+        int dev = 0, smem_sm = 0, regs_sm = 0;
+        cudaGetDevice(&dev);
+        cudaDeviceGetAttribute(&smem_sm, cudaDevAttrMaxSharedMemoryPerMultiprocessor, dev);
+        cudaDeviceGetAttribute(&regs_sm, cudaDevAttrMaxRegistersPerMultiprocessor, dev);
+        per_sm = 1;
+        if (cudaFuncGetAttributes(&fa, stage_tc_kernel<KP>) == cudaSuccess) {
+            const int by_smem = smem_sm / (int)(tc_smem_bytes(KP) + fa.sharedSizeBytes + 1024);
+            const int by_regs = regs_sm / (((fa.numRegs + 7) & ~7) * 128 * tc_q(KP));
+            per_sm = by_smem < by_regs ? by_smem : by_regs;
+        }
+        if (per_sm < 1) per_sm = 1;
+        if (per_sm > 4) per_sm = 4;  // 4 x 128 TMEM columns
+    }
+    const long long cap = (long long)sms * per_sm;
+    const unsigned grid = (unsigned)(nt < cap ? nt : cap);
+    stage_tc_kernel<KP><<<grid, 128 * tc_q(KP), tc_smem_bytes(KP), st>>>(g, in, out, mat, nt);
+    return cudaGetLastError() == cudaSuccess;
+}
+
+inline bool stage_tc_launch(const StageGeom &g, const void *src, void *dst, const uint8_t *mat, const DevConsts *, cudaStream_t st) {
+    static int sms = 0;
+    if (!sms) {
+        int dev = 0;
+        cudaGetDevice(&dev);
+        cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    }
     const int KP = tc_pad(g.K);
     const long long nt = (long long)((g.nb + 1) / 2) * g.ns * g.no;
     const uint64_t *in = (const uint64_t *)src;
     ulonglong2 *out = (ulonglong2 *)dst;
-    if (KP == 32) stage_tc_kernel<32><<<(unsigned)nt, TC_THREADS, tc_smem_bytes(32), st>>>(g, in, out, mat, dc);
-    else if (KP == 16) stage_tc_kernel<16><<<(unsigned)nt, TC_THREADS, tc_smem_bytes(16), st>>>(g, in, out, mat, dc);
-    else stage_tc_kernel<8><<<(unsigned)nt, TC_THREADS, tc_smem_bytes(8), st>>>(g, in, out, mat, dc);
-    return cudaGetLastError() == cudaSuccess;
+    if (KP == 32) return stage_tc_launch_kp<32>(g, in, out, mat, nt, sms, st);
+    if (KP == 16) return stage_tc_launch_kp<16>(g, in, out, mat, nt, sms, st);
+    return stage_tc_launch_kp<8>(g, in, out, mat, nt, sms, st);
 }
 
 }  // namespace oz
