@@ -97,6 +97,7 @@ __global__ void __launch_bounds__(128 * tc_q(KP), KP >= 32 ? 1 : 2) stage_tc_ker
     const uint32_t tmem = s_tmem;
     const uint32_t idesc = make_idesc(CFMT_S32, I8_S8, I8_S8, 128, NCOL);
     const uint32_t lane_taddr = tmem + ((uint32_t)((warp & 3) * 32) << 16);
+    const uint32_t full_addr = smem_u32(&bar_full[0]);
 
     // per-tile addressing: (valid, input base, output base, matrix base)
     auto locate = [&](long long t, bool &valid, long long &ib, long long &ob, const uint8_t *&mb) {
@@ -175,7 +176,7 @@ __global__ void __launch_bounds__(128 * tc_q(KP), KP >= 32 ? 1 : 2) stage_tc_ker
 
     auto epilogue = [&](int i) {  // a5: recombine digits, canonicalise, park residues of modulus i
         const int buf = i & 1;
-        mbar_wait(&bar_full[buf], (i >> 1) & 1);
+        mbar_wait_addr(full_addr + 8 * buf, (i >> 1) & 1);
         tc_fence_after();
         if (tid == 0 && (i + 2 < 12 || more)) {  // MMA i is complete: its matrix buffer takes modulus i+2 (or the
             const uint8_t *src = i + 2 < 12 ? matbase + (size_t)(i + 2) * MB : nmat + (size_t)(i - 10) * MB;  // next tile's)
@@ -249,7 +250,7 @@ __global__ void __launch_bounds__(128 * tc_q(KP), KP >= 32 ? 1 : 2) stage_tc_ker
 
     // ---- a6-a9: exact CRT, lift, pack; a12: store (the re thread stores even k, the im thread odd k)
     const int gexp = 53 + 52 - Tmax;
-#pragma unroll 1
+#pragma unroll 2
     for (int kk = 0; kk < JC; kk++) {
         const int k = q * JC + kk;
         uint64_t y;
