@@ -54,7 +54,7 @@ size_t ozfft_plan_device_bytes(ozfft_plan plan);
 int ozfft_exec_axis(ozfft_plan plan, int axis, const void *in, void *out, void *stream);
 /* Silicon-contract probe: D[128][n] (raw 32-bit accumulators) = A[128][kbytes] * B[n][kbytes]^T as chained
  * M=128 tcgen05.mma of K = 32 bytes each.  kind 0: f8f6f4 E4M3 -> f32; 1: f16 -> f32; 2: i8 (s8) -> s32;
- * 3: f16 with A fed from TMEM.  All pointers device.  n multiple of 16 in [16,256], kbytes multiple of 32. */
+ * 3: f16 with A fed from TMEM; 4: i8 (u8 x u8) -> s32.  All pointers device.  n multiple of 16 in [16,256], kbytes multiple of 32. */
 int ozfft_probe_mma(int kind, int n, int kbytes, const void *dA, const void *dB, void *dD, void *stream);
 
 #ifdef __cplusplus

@@ -25,6 +25,7 @@ struct DevConsts {
     uint32_t c36[12];    // 2^36 mod m
     uint32_t m2[12];     // 2 m
     uint32_t zC;         // round(2^149 / M): zhat = (umulhi(E >> 104, zC) + 2^12) >> 13
+    uint32_t phaseA[128];  // Phase-A constant matrix: 16 slice rows x 32 bytes in MMA operand order
 };
 
 // the same constants in the constant bank (uniform operands, no shared-memory loads); set by stage_tc_prepare
@@ -158,6 +159,8 @@ __device__ __forceinline__ void abs128(uint32_t *a, const uint32_t *x, uint32_t 
 // representative: m_k u_k == 0 mod M), quotient zhat = round(E/M) read off the top 30 bits of E (the lift of
 // PAPER.md:370 with the fraction taken from E itself), R = E - zhat M, two-sided centring.
 // r[0..3]: two's-complement limbs of R in [-M/2, M/2).
+__device__ __forceinline__ void crt_from_E(uint32_t e0, uint32_t e1, uint32_t e2, uint32_t e3, uint32_t e4, uint32_t *r);
+
 __device__ __forceinline__ void crt_limbs(const uint32_t *v, uint32_t *r) {
     uint64_t a0 = 0, a1 = 0, a2 = 0, a3 = 0;
 #pragma unroll
@@ -170,7 +173,22 @@ __device__ __forceinline__ void crt_limbs(const uint32_t *v, uint32_t *r) {
     a1 += a0 >> 32;
     a2 += a1 >> 32;
     a3 += a2 >> 32;
-    const uint32_t e0 = (uint32_t)a0, e1 = (uint32_t)a1, e2 = (uint32_t)a2, e3 = (uint32_t)a3, e4 = (uint32_t)(a3 >> 32);
+    crt_from_E((uint32_t)a0, (uint32_t)a1, (uint32_t)a2, (uint32_t)a3, (uint32_t)(a3 >> 32), r);
+}
+
+// Phase B (Alg. 2): deposit the 16 Phase-A slice sums P_s (each < 2^21) at byte offsets
+// 8s -- four 64-bit words of four slices each, one carry sweep -- giving E = sum_s P_s 256^s in 32-bit limbs.
+__device__ __forceinline__ void deposit_slices(const uint32_t *P, uint32_t *r) {
+    uint64_t w[4];
+#pragma unroll
+    for (int j = 0; j < 4; j++)
+        w[j] = (uint64_t)P[4 * j] + ((uint64_t)P[4 * j + 1] << 8) + ((uint64_t)P[4 * j + 2] << 16) + ((uint64_t)P[4 * j + 3] << 24);
+    const uint64_t t1 = (w[0] >> 32) + w[1], t2 = (t1 >> 32) + w[2], t3 = (t2 >> 32) + w[3];
+    crt_from_E((uint32_t)w[0], (uint32_t)t1, (uint32_t)t2, (uint32_t)t3, (uint32_t)(t3 >> 32), r);
+}
+
+// lift and centring from the limbs of E (< 2^134): see crt_limbs
+__device__ __forceinline__ void crt_from_E(uint32_t e0, uint32_t e1, uint32_t e2, uint32_t e3, uint32_t e4, uint32_t *r) {
     const uint32_t T = __funnelshift_r(e3, e4, 8);  // E >> 104
     const uint32_t z = (__umulhi(T, kc.zC) + (1u << 12)) >> 13;
     uint64_t p0 = (uint64_t)z * kc.M[0];

@@ -95,6 +95,18 @@ void fill_consts(DevConsts &c) {
         if (rem * 2 >= C.M) q++;
         c.zC = (uint32_t)q;
     }
+    {  // Phase-A matrix, two-limb shifted-column form: residue v = v0 + 256 v1 sits in operand bytes (2k, 2k+1);
+       // row s holds byte s of u_k against v0 and byte s-1 against v1.  Operand order [chunk][row][16 B].
+        uint8_t *pa = (uint8_t *)c.phaseA;
+        memset(pa, 0, 512);
+        for (int s = 0; s < 16; s++)
+            for (int k = 0; k < R_MOD; k++)
+                for (int l = 0; l < 2; l++) {
+                    const int sh = s - l, kap = 2 * k + l;
+                    const uint8_t b = sh < 0 ? 0 : (uint8_t)(C.u[k] >> (8 * sh));
+                    pa[(kap / 16) * 256 + s * 16 + kap % 16] = b;
+                }
+    }
     for (int l = 0; l < 4; l++) {
         c.M[l] = (uint32_t)(C.M >> (32 * l));
         c.Mh[l] = (uint32_t)(C.Mhalf >> (32 * l));

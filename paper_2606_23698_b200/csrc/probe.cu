@@ -10,6 +10,7 @@ using namespace oz;
 
 // A: [128][kb] bytes row-major (K-major), B: [n][kb] bytes row-major, D: [128][n] raw 32-bit accumulators.
 // kind: 0 f8f6f4(E4M3,f32) 1 f16(f16,f32) 2 i8(s8,s32) 3 f16 with A staged through TMEM (tcgen05.st + .ts MMA)
+//       4 i8(u8 x u8,s32)
 __global__ void __launch_bounds__(128, 1) probe_kernel(int kind, int n, int kb, const uint8_t *A, const uint8_t *B, uint32_t *D) {
     extern __shared__ __align__(128) uint8_t smem[];
     __shared__ uint64_t bar;
@@ -45,15 +46,15 @@ __global__ void __launch_bounds__(128, 1) probe_kernel(int kind, int n, int kb, 
         tc_fence_after();
     }
     if (tid == 0) {
-        const uint32_t cf = kind == 2 ? CFMT_S32 : CFMT_F32;
-        const uint32_t fmt = kind == 0 ? F8_E4M3 : (kind == 2 ? I8_S8 : F16_F16);
+        const uint32_t cf = (kind == 2 || kind == 4) ? CFMT_S32 : CFMT_F32;
+        const uint32_t fmt = kind == 0 ? F8_E4M3 : (kind == 2 ? I8_S8 : (kind == 4 ? I8_U8 : F16_F16));
         const uint32_t idesc = make_idesc(cf, fmt, fmt, 128, n);
         for (int ks = 0; ks < kb / 32; ks++) {
             uint64_t ad = make_sdesc(smem_u32(sA) + ks * 2 * 128 * 16, 128 * 16, 128);
             uint64_t bd = make_sdesc(smem_u32(sB) + ks * 2 * n * 16, n * 16, 128);
             if (kind == 0) mma_f8f6f4_ss(tmem, ad, bd, idesc, ks > 0);
             else if (kind == 1) mma_f16_ss(tmem, ad, bd, idesc, ks > 0);
-            else if (kind == 2) mma_i8_ss(tmem, ad, bd, idesc, ks > 0);
+            else if (kind == 2 || kind == 4) mma_i8_ss(tmem, ad, bd, idesc, ks > 0);
             else mma_f16_ts(tmem, tmem + 256 + ks * 8, bd, idesc, ks > 0);
         }
         tc_commit(&bar);
@@ -74,7 +75,7 @@ __global__ void __launch_bounds__(128, 1) probe_kernel(int kind, int n, int kb, 
 }  // namespace
 
 extern "C" int ozfft_probe_mma(int kind, int n, int kbytes, const void *dA, const void *dB, void *dD, void *stream) {
-    if (kind < 0 || kind > 3 || n < 16 || n > 256 || (n % 16) || kbytes < 32 || (kbytes % 32)) return OZFFT_EINVAL;
+    if (kind < 0 || kind > 4 || n < 16 || n > 256 || (n % 16) || kbytes < 32 || (kbytes % 32)) return OZFFT_EINVAL;
     size_t sm = (size_t)(128 + n) * kbytes;
     if (sm > 200 * 1024) return OZFFT_EINVAL;
     cudaFuncSetAttribute(probe_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);

@@ -21,15 +21,14 @@ namespace oz {
 
 // threads per CTA = 128 * Q: Q thread groups share each MMA row and split its contraction elements / outputs
 __host__ __device__ constexpr int tc_q(int) { return 4; }
-constexpr int TC_TMEM_COLS = 128;
+constexpr int TC_TMEM_COLS = 256;  // [0,128): stage accumulators (2 x 64); Phase-A sums alternate [128,256) / [0,128)
 
 // bytes of one modulus' matrix planes for padded length KP: rows n = 2k + d (d = digit 0/1), 4 KP bytes each,
 // stored in the canonical K-major no-swizzle core-matrix order [chunk = byte/16][row n][16 B]
 __host__ __device__ constexpr int tc_mat_bytes(int KP) { return 8 * KP * KP; }
 __host__ __device__ constexpr int tc_pad(int K) { return K < 8 ? 8 : K; }
-__host__ __device__ constexpr int tc_rs_stride(int KP) { return KP * 24 + 8; }
 __host__ __device__ constexpr size_t tc_smem_bytes(int KP) {
-    return 2 * (size_t)128 * 4 * KP + 2 * (size_t)tc_mat_bytes(KP) + (size_t)128 * tc_rs_stride(KP);
+    return 2 * (size_t)128 * 4 * KP + 2 * (size_t)tc_mat_bytes(KP) + (size_t)KP * 4096 + 512;
 }
 
 // host: digit planes of matrix set (K, fusedN) for all matrix ids and moduli: [mid][i][tc_mat_bytes]
@@ -70,13 +69,16 @@ __global__ void __launch_bounds__(128 * tc_q(KP), KP >= 32 ? 1 : 2) stage_tc_ker
     constexpr int JC = KP / Q;         // contraction elements (and outputs) per thread
     constexpr int ABYTES = 128 * 4 * KP;
     constexpr int MB = tc_mat_bytes(KP);
-    constexpr int RS = tc_rs_stride(KP);
+    constexpr int NB = JC / 2;         // Phase-A batches: 2 outputs per thread = 8 MMAs of N = 16 each
     constexpr int NCOL = 2 * KP;       // accumulator columns per modulus
     extern __shared__ __align__(128) uint8_t smem[];
-    __shared__ __align__(8) uint64_t bar_full[2], bar_load[2];
+    __shared__ __align__(8) uint64_t bar_full[2], bar_load[2], bar_pa[2];
     __shared__ uint32_t s_tmem;
     __shared__ int s_tmax[2][64], s_flag[2][64];
     uint8_t *sA = smem, *sB = smem + 2 * ABYTES, *sR = smem + 2 * ABYTES + 2 * MB;
+    uint8_t *sPA = sR + KP * 4096;  // Phase-A constant matrix (operand order), 512 B
+    // sR: residue store = Phase-A data operand: per output k a [2 chunks][128 rows][16 B] tile, residue i of row r at
+    // k*4096 + (i/8)*2048 + r*16 + (i%8)*2 (u16 little endian = the two limbs v0, v1 of PAPER.md:759)
 
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     const int row = (warp & 3) * 32 + lane, q = warp >> 2;  // q < Q
@@ -85,10 +87,12 @@ __global__ void __launch_bounds__(128 * tc_q(KP), KP >= 32 ? 1 : 2) stage_tc_ker
     const int nbt = (g.nb + 1) >> 1;
 
     if (tid < 64) { s_tmax[0][tid] = s_tmax[1][tid] = -100000; s_flag[0][tid] = s_flag[1][tid] = 0; }
+    if (tid < 128) ((uint32_t *)sPA)[tid] = kc.phaseA[tid];
     if (warp == 0) tmem_alloc<TC_TMEM_COLS>(&s_tmem);
     if (tid == 0) {
         mbar_init(&bar_full[0], 1); mbar_init(&bar_full[1], 1);
         mbar_init(&bar_load[0], 1); mbar_init(&bar_load[1], 1);
+        mbar_init(&bar_pa[0], 1); mbar_init(&bar_pa[1], 1);
         mbar_fence_init();
     }
     tc_fence_before();
@@ -135,6 +139,7 @@ __global__ void __launch_bounds__(128 * tc_q(KP), KP >= 32 ? 1 : 2) stage_tc_ker
     uint64_t bits[JC];
     load_inputs(colvalid, ibase, bits);
     int tpar = 0;
+    uint32_t pa_phase = 0;  // parity of the next completion of each Phase-A barrier
 
 #pragma unroll 1
     for (; tile < ntiles; tile += gridDim.x, tpar ^= 1) {
@@ -174,6 +179,7 @@ __global__ void __launch_bounds__(128 * tc_q(KP), KP >= 32 ? 1 : 2) stage_tc_ker
     if (more) locate(ntile, nvalid, nib, nob, nmat);
     load_inputs(more && nvalid, nib, bits);
 
+    uint32_t held[JC];  // residues of the even modulus of a pair, stored together with the odd one
     auto epilogue = [&](int i) {  // a5: recombine digits, canonicalise, park residues of modulus i
         const int buf = i & 1;
         mbar_wait_addr(full_addr + 8 * buf, (i >> 1) & 1);
@@ -193,7 +199,9 @@ __global__ void __launch_bounds__(128 * tc_q(KP), KP >= 32 ? 1 : 2) stage_tc_ker
 #pragma unroll
         for (int kk = 0; kk < JC; kk++) {  // residue left in [0, 2m): any representative serves the CRT
             const uint32_t v = (uint32_t)((int)r[2 * kk + 1] * 128 + (int)r[2 * kk]) + off;
-            *(uint16_t *)(sR + row * RS + (q * JC + kk) * 24 + 2 * i) = (uint16_t)(v + __umulhi(v, mu) * negm);
+            const uint32_t res = v + __umulhi(v, mu) * negm;
+            if (i & 1) *(uint32_t *)(sR + (q * JC + kk) * 4096 + (i >> 3) * 2048 + row * 16 + ((i - 1) & 7) * 2) = held[kk] | (res << 16);
+            else held[kk] = res;
         }
         tc_fence_before();
     };
@@ -248,34 +256,65 @@ __global__ void __launch_bounds__(128 * tc_q(KP), KP >= 32 ? 1 : 2) stage_tc_ker
     }
     epilogue(11);
 
-    // ---- a6-a9: exact CRT, lift, pack; a12: store (the re thread stores even k, the im thread odd k)
-    const int gexp = 53 + 52 - Tmax;
-#pragma unroll 2
-    for (int kk = 0; kk < JC; kk++) {
-        const int k = q * JC + kk;
-        uint64_t y;
-        if (flag & 2) y = 0x7FF8000000000000ull;
-        else if (flag == 0) y = 0;
-        else {
-            uint32_t v[12];
-            const uint2 *p = (const uint2 *)(sR + row * RS + k * 24);
+    // ---- a6: Phase A on the tensor core (Eq. 20, two-limb form 759-764): for each output k,
+    // P[row][s] = sum over the 24 residue-limb bytes of the row x the slice matrix; u8 x u8 -> s32, N = 16.
+    // Batch b covers outputs k = q'*JC + 2b + e (q' < 4, e < 2): thread group q' reads its 32 columns at q'*32.
+    fence_async_smem();
+    tc_fence_before();
+    __syncthreads();
+    auto issue_pa = [&](int b) {
+        const uint32_t idesc_pa = make_idesc(CFMT_S32, I8_U8, I8_U8, 128, 16);
+        const uint64_t bd = make_sdesc(smem_u32(sPA), 16 * 16, 128);
+        const uint32_t dcol = tmem + ((b + 1) & 1) * 128;
 #pragma unroll
-            for (int t = 0; t < 3; t++) {
-                const uint2 u = p[t];
-                v[4 * t] = u.x & 0xFFFF; v[4 * t + 1] = u.x >> 16;
-                v[4 * t + 2] = u.y & 0xFFFF; v[4 * t + 3] = u.y >> 16;
+        for (int qq = 0; qq < Q; qq++)
+#pragma unroll
+            for (int e = 0; e < 2; e++) {
+                const int k = qq * JC + 2 * b + e;
+                mma_i8_ss(dcol + qq * 32 + e * 16, make_sdesc(smem_u32(sR) + k * 4096, 128 * 16, 128), bd, idesc_pa, 0);
             }
-            uint32_t R[4];
-            crt_limbs(v, R);
-            y = pack_limbs(R, gexp);
+        tc_commit(&bar_pa[b & 1]);
+    };
+    if (tid == 0) {
+        tc_fence_after();
+        issue_pa(0);
+        if (NB > 1) issue_pa(1);
+    }
+    // ---- a7-a9: Phase B deposits, lift, pack; a12: store (the re thread stores even k, the im thread odd k)
+    const int gexp = 53 + 52 - Tmax;
+#pragma unroll 1
+    for (int b = 0; b < NB; b++) {
+        mbar_wait(&bar_pa[b & 1], (pa_phase >> (b & 1)) & 1);
+        pa_phase ^= 1u << (b & 1);
+        tc_fence_after();
+        uint32_t P[32];
+        tmem_ld_x32(lane_taddr + ((b + 1) & 1) * 128 + q * 32, P);
+        tmem_ld_wait();
+        tc_fence_before();
+        __syncthreads();
+        if (tid == 0 && b + 2 < NB) {
+            tc_fence_after();
+            issue_pa(b + 2);
         }
-        const uint32_t plo = __shfl_xor_sync(0xFFFFFFFFu, (uint32_t)y, 1), phi = __shfl_xor_sync(0xFFFFFFFFu, (uint32_t)(y >> 32), 1);
-        const uint64_t yp = ((uint64_t)phi << 32) | plo;
-        if (colvalid && k < K && (k & 1) == part) {
-            ulonglong2 o;
-            o.x = part ? yp : y;
-            o.y = part ? y : yp;
-            out[obase + k * g.ko] = o;
+#pragma unroll
+        for (int e = 0; e < 2; e++) {
+            const int k = q * JC + 2 * b + e;
+            uint64_t y;
+            if (flag & 2) y = 0x7FF8000000000000ull;
+            else if (flag == 0) y = 0;
+            else {
+                uint32_t R[4];
+                deposit_slices(P + 16 * e, R);
+                y = pack_limbs(R, gexp);
+            }
+            const uint32_t plo = __shfl_xor_sync(0xFFFFFFFFu, (uint32_t)y, 1), phi = __shfl_xor_sync(0xFFFFFFFFu, (uint32_t)(y >> 32), 1);
+            const uint64_t yp = ((uint64_t)phi << 32) | plo;
+            if (colvalid && k < K && (k & 1) == part) {
+                ulonglong2 o;
+                o.x = part ? yp : y;
+                o.y = part ? y : yp;
+                out[obase + k * g.ko] = o;
+            }
         }
     }
     colvalid = nvalid; ibase = nib; obase = nob; matbase = nmat;
@@ -309,7 +348,7 @@ inline bool stage_tc_launch_kp(const StageGeom &g, const uint64_t *in, ulonglong
             per_sm = by_smem < by_regs ? by_smem : by_regs;
         }
         if (per_sm < 1) per_sm = 1;
-        if (per_sm > 4) per_sm = 4;  // 4 x 128 TMEM columns
+        if (per_sm > 2) per_sm = 2;  // 2 x 256 TMEM columns
     }
     const long long cap = (long long)sms * per_sm;
     const unsigned grid = (unsigned)(nt < cap ? nt : cap);

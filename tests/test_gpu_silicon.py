@@ -59,3 +59,14 @@ def test_f16_phase_a_contract(kind):
     want = V.astype(np.int64) @ U.astype(np.int64).T
     assert want.max() == 12 * 2038 * 255
     assert np.array_equal(D.astype(np.int64), want)
+
+
+def test_u8_phase_a_two_limb_contract():
+    """Phase A in the two-limb shifted-column form: u8 residue limbs x u8 slices -> s32."""
+    rng = np.random.default_rng(4)
+    A = rng.integers(0, 256, (128, 32), dtype=np.uint8)
+    B = rng.integers(0, 256, (16, 32), dtype=np.uint8)
+    A[0] = 255
+    B[0] = 255
+    D = _probe(4, A, B)
+    assert np.array_equal(D, A.astype(np.int64) @ B.astype(np.int64).T) and D.max() == 32 * 255 * 255
