@@ -86,6 +86,22 @@ class ClockSampler:
                 "samples": len(sm)}
 
 
+def max_over_ranks(values, device="cpu"):
+    """element-wise MAX over the ranks of the default process group (identity when not initialised):
+    every multi-GPU number is the slowest rank's (timed on the device)."""
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor(list(values), dtype=torch.float64, device=device)
+    if dist.is_available() and dist.is_initialized() and dist.get_world_size() > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return [float(v) for v in t]
+
+
+# DRAM bytes of one stage launch at 1024^3 from the committed ncu capture (profiles/r1_final.md):
+# dram__bytes_read.sum + dram__bytes_write.sum = 17.20 + 17.14 GB against 34.36 GB algorithmic
+NCU_TRAFFIC_PER_LAUNCH = {1024: 3.434e10}
+
+
 def cpu_oracle_sample(size, pencils):
     """Times the oracle (as it stands, direct exact-integer route) on `pencils` length-`size` pencils of the
     workload's own data; returns (seconds, threads)."""
@@ -222,10 +238,7 @@ def run_ours(args):
     except Exception as ex:  # out of memory at the largest size is not fatal for the bench line
         cufft_ms = None
 
-    t_max = torch.tensor([ms_step, e2e_ms], dtype=torch.float64, device="cuda")
-    if world > 1:
-        dist.all_reduce(t_max, op=dist.ReduceOp.MAX)
-    ms_step_max, e2e_ms_max = float(t_max[0]), float(t_max[1])
+    ms_step_max, e2e_ms_max = max_over_ranks([ms_step, e2e_ms], device="cuda")
 
     if rank == 0:
         peak, peak_src = peaks()
@@ -244,12 +257,15 @@ def run_ours(args):
             "hbm_roof": {"alg_bytes": 96.0 * n_tot if launches == 6 else alg_bytes_launch * launches / 2,
                          "roof_ms_at_measured_peak": 96.0 * n_tot / (peak * 1e9) * 1e3, "frac_of_roof": (96.0 * n_tot / (peak * 1e9) * 1e3) / ms_step},
             "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                         "traffic": None, "kernel": "stage kernel (all launches of a transform are this kernel)",
+                         "traffic": NCU_TRAFFIC_PER_LAUNCH.get(size), "kernel": "stage kernel (all launches of a transform are this kernel)",
                          "peak_source": peak_src, "alg_bytes_per_launch": alg_bytes_launch, "launch_ms": launch_ms},
             "clocks": clocks,
             "e2e": {"value": world * flops(n_tot) / (e2e_ms_max * 1e-3) / 1e9, "unit": "GFLOP/s", "ms": e2e_ms_max,
                     "h2d_bytes_per_step": nbytes, "d2h_bytes_per_step": nbytes, "steps": e2e_steps},
             "gpu_launches": launches * args.steps,
+            "integer_issue": {"n_out": 2 * launches * n_tot, "peak_thread_inst_per_s": 148 * 128 * 1.965e9,
+                              "note": "the path is bound by SIMT integer issue (PAPER.md:452); measured thread "
+                                      "instructions per output-equivalent and issue-slot use are in profiles/"},
             "context": {"cufft_z2z_ms": cufft_ms, "paper_projection_ms_B300": [63, 87], "paper_projection_ms_B200": [70, 96],
                         "paper_hbm_roof_ms": 12.9},
         }
