@@ -28,7 +28,7 @@ constexpr int TC_TMEM_COLS = 256;  // [0,128): stage accumulators (2 x 64); Phas
 __host__ __device__ constexpr int tc_mat_bytes(int KP) { return 8 * KP * KP; }
 __host__ __device__ constexpr int tc_pad(int K) { return K < 8 ? 8 : K; }
 __host__ __device__ constexpr size_t tc_smem_bytes(int KP) {
-    return 2 * (size_t)128 * 4 * KP + 2 * (size_t)tc_mat_bytes(KP) + (size_t)KP * 4096 + 512;
+    return 2 * (size_t)128 * 4 * KP + 4 * (size_t)tc_mat_bytes(KP) + (size_t)KP * 4096 + 512;
 }
 
 // host: digit planes of matrix set (K, fusedN) for all matrix ids and moduli: [mid][i][tc_mat_bytes]
@@ -75,7 +75,7 @@ __global__ void __launch_bounds__(128 * tc_q(KP), KP >= 32 ? 1 : 2) stage_tc_ker
     __shared__ __align__(8) uint64_t bar_full[2], bar_load[2], bar_pa[2];
     __shared__ uint32_t s_tmem;
     __shared__ int s_tmax[2][64], s_flag[2][64];
-    uint8_t *sA = smem, *sB = smem + 2 * ABYTES, *sR = smem + 2 * ABYTES + 2 * MB;
+    uint8_t *sA = smem, *sB = smem + 2 * ABYTES, *sR = smem + 2 * ABYTES + 4 * MB;
     uint8_t *sPA = sR + KP * 4096;  // Phase-A constant matrix (operand order), 512 B
     // sR: residue store = Phase-A data operand: per output k a [2 chunks][128 rows][16 B] tile, residue i of row r at
     // k*4096 + (i/8)*2048 + r*16 + (i%8)*2 (u16 little endian = the two limbs v0, v1 of PAPER.md:759)
@@ -130,16 +130,18 @@ __global__ void __launch_bounds__(128 * tc_q(KP), KP >= 32 ? 1 : 2) stage_tc_ker
     long long ibase, obase;
     const uint8_t *matbase;
     locate(tile, colvalid, ibase, obase, matbase);
-    if (tid == 0) {  // matrix planes of moduli 0 and 1 of the first tile
-        mbar_expect_tx(&bar_load[0], MB);
-        bulk_g2s(sB, matbase, MB, &bar_load[0]);
-        mbar_expect_tx(&bar_load[1], MB);
-        bulk_g2s(sB + MB, matbase + MB, MB, &bar_load[1]);
+    if (tid == 0) {  // matrix planes of modulus pairs 0 and 1 of the first tile
+        mbar_expect_tx(&bar_load[0], 2 * MB);
+        bulk_g2s(sB, matbase, 2 * MB, &bar_load[0]);
+        mbar_expect_tx(&bar_load[1], 2 * MB);
+        bulk_g2s(sB + 2 * MB, matbase + 2 * MB, 2 * MB, &bar_load[1]);
     }
     uint64_t bits[JC];
     load_inputs(colvalid, ibase, bits);
     int tpar = 0;
     uint32_t pa_phase = 0;  // parity of the next completion of each Phase-A barrier
+    uint32_t full_ph = 0, load_ph = 0;  // same for the MMA-done and matrix-landed barriers (bit = buffer)
+    const uint32_t nm7 = part ? 0x7F7F7F7Fu : 0u, nm1 = part ? 0x01010101u : 0u, nm8 = part ? 0x80808080u : 0u;
 
 #pragma unroll 1
     for (; tile < ntiles; tile += gridDim.x, tpar ^= 1) {
@@ -179,82 +181,91 @@ __global__ void __launch_bounds__(128 * tc_q(KP), KP >= 32 ? 1 : 2) stage_tc_ker
     if (more) locate(ntile, nvalid, nib, nob, nmat);
     load_inputs(more && nvalid, nib, bits);
 
-    uint32_t held[JC];  // residues of the even modulus of a pair, stored together with the odd one
-    auto epilogue = [&](int i) {  // a5: recombine digits, canonicalise, park residues of modulus i
-        const int buf = i & 1;
-        mbar_wait_addr(full_addr + 8 * buf, (i >> 1) & 1);
+    // Moduli go through the pipeline in pairs (one barrier, one fence and one commit per pair).
+    auto epilogue = [&](int p) {  // a5: recombine digits, reduce, park the residues of moduli 2p and 2p+1
+        const int buf = p & 1;
+        mbar_wait_addr(full_addr + 8 * buf, (full_ph >> buf) & 1);
+        full_ph ^= 1u << buf;
         tc_fence_after();
-        if (tid == 0 && (i + 2 < 12 || more)) {  // MMA i is complete: its matrix buffer takes modulus i+2 (or the
-            const uint8_t *src = i + 2 < 12 ? matbase + (size_t)(i + 2) * MB : nmat + (size_t)(i - 10) * MB;  // next tile's)
-            mbar_expect_tx(&bar_load[buf], MB);
-            bulk_g2s(sB + buf * MB, src, MB, &bar_load[buf]);
+        if (tid == 0 && (p + 2 < 6 || more)) {  // MMAs of pair p are complete: their matrix buffer takes pair p+2
+            const uint8_t *src = p + 2 < 6 ? matbase + (size_t)(p + 2) * 2 * MB : nmat + (size_t)(p - 4) * 2 * MB;  // or the next tile's
+            mbar_expect_tx(&bar_load[buf], 2 * MB);
+            bulk_g2s(sB + buf * 2 * MB, src, 2 * MB, &bar_load[buf]);
         }
-        uint32_t r[2 * JC];
-        const uint32_t ta = lane_taddr + buf * 64 + 2 * q * JC;
-        if constexpr (JC == 8) tmem_ld_x16(ta, r);
-        else if constexpr (JC == 4) tmem_ld_x8(ta, r);
-        else tmem_ld_x4(ta, r);
+        uint32_t r0[2 * JC], r1[2 * JC];
+        const uint32_t ta = lane_taddr + buf * 128 + 2 * q * JC;
+        if constexpr (JC == 8) { tmem_ld_x16(ta, r0); tmem_ld_x16(ta + 64, r1); }
+        else if constexpr (JC == 4) { tmem_ld_x8(ta, r0); tmem_ld_x8(ta + 64, r1); }
+        else { tmem_ld_x4(ta, r0); tmem_ld_x4(ta + 64, r1); }
         tmem_ld_wait();
-        const uint32_t negm = 0u - kc.m[i], mu = kc.mu[i], off = kc.offtc[i];
+        const int i0 = 2 * p;
+        const uint32_t negm0 = 0u - kc.m[i0], mu0 = kc.mu[i0], off0 = kc.offtc[i0];
+        const uint32_t negm1 = 0u - kc.m[i0 + 1], mu1 = kc.mu[i0 + 1], off1 = kc.offtc[i0 + 1];
+        uint8_t *dst = sR + (q * JC) * 4096 + (i0 >> 3) * 2048 + row * 16 + (i0 & 7) * 2;
 #pragma unroll
-        for (int kk = 0; kk < JC; kk++) {  // residue left in [0, 2m): any representative serves the CRT
-            const uint32_t v = (uint32_t)((int)r[2 * kk + 1] * 128 + (int)r[2 * kk]) + off;
-            const uint32_t res = v + __umulhi(v, mu) * negm;
-            if (i & 1) *(uint32_t *)(sR + (q * JC + kk) * 4096 + (i >> 3) * 2048 + row * 16 + ((i - 1) & 7) * 2) = held[kk] | (res << 16);
-            else held[kk] = res;
+        for (int kk = 0; kk < JC; kk++) {  // residues left in [0, 2m): any representative serves the CRT
+            const uint32_t v0 = (uint32_t)((int)r0[2 * kk + 1] * 128 + (int)r0[2 * kk]) + off0;
+            const uint32_t v1 = (uint32_t)((int)r1[2 * kk + 1] * 128 + (int)r1[2 * kk]) + off1;
+            const uint32_t a = v0 + __umulhi(v0, mu0) * negm0, b = v1 + __umulhi(v1, mu1) * negm1;
+            *(uint32_t *)(dst + kk * 4096) = a | (b << 16);
         }
         tc_fence_before();
     };
 
 #pragma unroll 1
-    for (int i = 0; i < 12; i++) {
-        // ---- a3 (second half): residues mod m_i of own elements -> digit bytes (x0, x1) per element
-        const uint32_t mu = kc.mu[i], negm = 0u - kc.m[i], m2 = kc.m2[i], c18 = kc.c18[i], c36 = kc.c36[i];
-        uint32_t w[JC / 2];
+    for (int p = 0; p < 6; p++) {
+        // the data operand is single-buffered: the MMAs of pair p-1 (issued before the previous epilogue) must be done
+        if (p > 0) mbar_wait_addr(full_addr + 8 * ((p - 1) & 1), (full_ph >> ((p - 1) & 1)) & 1);
 #pragma unroll
-        for (int jj = 0; jj < JC; jj++) {
-            uint32_t rr = x0[jj] + x1[jj] * c18 + x2[jj] * c36;  // < 2^30
-            rr += __umulhi(rr, mu) * negm;                        // in [0, 2m)
-            if ((negmask >> jj) & 1) rr = m2 - rr;                // -x: in (0, 2m]
-            const uint32_t hw = rr + (rr & 0xFF80u);              // digits x0 = rr & 127, x1 = rr >> 7 as two bytes
-            if (jj & 1) w[jj >> 1] |= hw << 16;
-            else w[jj >> 1] = hw;
-        }
-        // own digits go to the first half of the own row, the partner's (negated for the re row) to the second
-        uint8_t *A = sA + (i & 1) * ABYTES;
+        for (int h2 = 0; h2 < 2; h2++) {
+            // ---- a3 (second half): residues mod m_i of own elements -> digit bytes (x0, x1) per element
+            const int i = 2 * p + h2;
+            const uint32_t mu = kc.mu[i], negm = 0u - kc.m[i], m2 = kc.m2[i], c18 = kc.c18[i], c36 = kc.c36[i];
+            uint32_t w[JC / 2], o[JC / 2];
 #pragma unroll
-        for (int h = 0; h < 2; h++) {
-            uint32_t o[JC / 2];
-#pragma unroll
-            for (int t = 0; t < JC / 2; t++) {
-                const uint32_t pw = __shfl_xor_sync(0xFFFFFFFFu, w[t], 1);
-                o[t] = h == 0 ? w[t] : (part == 0 ? neg_bytes(pw) : pw);
+            for (int jj = 0; jj < JC; jj++) {
+                uint32_t rr = x0[jj] + x1[jj] * c18 + x2[jj] * c36;  // < 2^30
+                rr += __umulhi(rr, mu) * negm;                        // in [0, 2m)
+                if ((negmask >> jj) & 1) rr = m2 - rr;                // -x: in (0, 2m]
+                const uint32_t hw = rr + (rr & 0xFF80u);              // digits x0 = rr & 127, x1 = rr >> 7 as two bytes
+                if (jj & 1) w[jj >> 1] |= hw << 16;
+                else w[jj >> 1] = hw;
             }
-            const int kap = h * 2 * KP + q * JC * 2;  // first contraction byte this thread writes
-            uint8_t *dst = A + (kap >> 4) * (128 * 16) + row * 16 + (kap & 15);
-            if constexpr (JC == 8) *(uint4 *)dst = make_uint4(o[0], o[1], o[2], o[3]);
-            else if constexpr (JC == 4) *(uint2 *)dst = make_uint2(o[0], o[1]);
-            else *(uint32_t *)dst = o[0];
+            // own digits: first half of the own row; second half of the partner row (row^1), negated when this is
+            // the im thread (the re row holds [x_R ; -x_I], the im row [x_I ; x_R])
+#pragma unroll
+            for (int t = 0; t < JC / 2; t++) o[t] = ((w[t] ^ nm7) + nm1) ^ nm8;
+            uint8_t *A = sA + h2 * ABYTES;
+            const int kap = q * JC * 2;  // first contraction byte of this thread within a half
+            uint8_t *d0 = A + (kap >> 4) * (128 * 16) + row * 16 + (kap & 15);
+            uint8_t *d1 = A + ((2 * KP + kap) >> 4) * (128 * 16) + (row ^ 1) * 16 + (kap & 15);
+            if constexpr (JC == 8) { *(uint4 *)d0 = make_uint4(w[0], w[1], w[2], w[3]); *(uint4 *)d1 = make_uint4(o[0], o[1], o[2], o[3]); }
+            else if constexpr (JC == 4) { *(uint2 *)d0 = make_uint2(w[0], w[1]); *(uint2 *)d1 = make_uint2(o[0], o[1]); }
+            else { *(uint32_t *)d0 = w[0]; *(uint32_t *)d1 = o[0]; }
         }
         fence_async_smem();
         tc_fence_before();
         __syncthreads();
-        // ---- a4: residue DFT of modulus i on the tensor core
+        // ---- a4: residue DFTs of moduli 2p, 2p+1 on the tensor core
         if (tid == 0) {
             tc_fence_after();
-            mbar_wait(&bar_load[i & 1], (i >> 1) & 1);
-            const uint32_t a0 = smem_u32(A), b0 = smem_u32(sB + (i & 1) * MB);
+            mbar_wait(&bar_load[p & 1], (load_ph >> (p & 1)) & 1);
+            load_ph ^= 1u << (p & 1);
 #pragma unroll
-            for (int ks = 0; ks < KP / 8; ks++) {
-                const uint64_t ad = make_sdesc(a0 + ks * 2 * 128 * 16, 128 * 16, 128);
-                const uint64_t bd = make_sdesc(b0 + ks * 2 * NCOL * 16, NCOL * 16, 128);
-                mma_i8_ss(tmem + (i & 1) * 64, ad, bd, idesc, ks > 0);
+            for (int h2 = 0; h2 < 2; h2++) {
+                const uint32_t a0 = smem_u32(sA + h2 * ABYTES), b0 = smem_u32(sB + (p & 1) * 2 * MB + h2 * MB);
+#pragma unroll
+                for (int ks = 0; ks < KP / 8; ks++) {
+                    const uint64_t ad = make_sdesc(a0 + ks * 2 * 128 * 16, 128 * 16, 128);
+                    const uint64_t bd = make_sdesc(b0 + ks * 2 * NCOL * 16, NCOL * 16, 128);
+                    mma_i8_ss(tmem + (p & 1) * 128 + h2 * 64, ad, bd, idesc, ks > 0);
+                }
             }
-            tc_commit(&bar_full[i & 1]);
+            tc_commit(&bar_full[p & 1]);
         }
-        if (i > 0) epilogue(i - 1);
+        if (p > 0) epilogue(p - 1);
     }
-    epilogue(11);
+    epilogue(5);
 
     // ---- a6: Phase A on the tensor core (Eq. 20, two-limb form 759-764): for each output k,
     // P[row][s] = sum over the 24 residue-limb bytes of the row x the slice matrix; u8 x u8 -> s32, N = 16.
