@@ -3,12 +3,17 @@
 // Tile: 64 columns.  MMA row r (= TMEM lane r) = (column r/2, part r&1): the re row holds the digits of
 // [x_R ; -x_I], the im row those of [x_I ; x_R], so ONE matrix operand [a_R ; a_I] yields both parts
 // (direct 4-product complex form).
-// Digits (base 128, from canonical residues, PAPER.md:113 layout is the builder's): x = x0 + 128 x1,
-// a = a0 + 128 a1, a' = 128 a mod m = a'0 + 128 a'1, so  a x == (a0 x0 + a'0 x1) + 128 (a1 x0 + a'1 x1) (mod m):
-// two s32 accumulators per output and modulus, contraction over (half, j, digit) = 4 K bytes.
-// Per modulus i: deconstruct digits -> SMEM operand (double buffered) -> tcgen05.mma into TMEM (double
-// buffered) while the SIMT epilogue of modulus i-1 canonicalises its accumulators into the residue store;
-// matrix planes arrive by TMA bulk copy one modulus ahead.  After 12 moduli: exact CRT + lift + pack.
+// Digits (PAPER.md:113 leaves the layout to the builder): every residue is kept as a representative r in
+// [0, 2m] (< 2^12) whose two bytes ARE the digits, x = x0 + 256 x1 (u8, u8 <= 15); -x is 2m - r, so all
+// digits are unsigned.  Matrix entries a and a' = 256 a mod m split the same way, and
+//   a x == (a0 x0 + a'0 x1) + 256 (a1 x0 + a'1 x1) (mod m):
+// two s32 accumulators (u8 x u8 products) per output and modulus, contraction over (half, j, digit) = 4 K bytes,
+// lo + 256 hi < 2^26.
+// Per modulus pair: deconstruct digits -> SMEM operand -> tcgen05.mma kind::i8 into TMEM (double buffered)
+// while the SIMT epilogue of the previous pair reduces its accumulators into the residue store; matrix planes
+// arrive by TMA bulk copy one pair ahead.  The residue store is the data operand of Phase A (tc-CRT):
+// a second kind::i8 MMA against the byte slices of the CRT idempotents; Phase B deposits the slice sums,
+// lifts (mod M, two-sided) and packs once to fp64.  CTAs are persistent and prefetch the next tile's inputs.
 #pragma once
 #include <vector>
 
@@ -45,10 +50,10 @@ inline void build_mat_tc(std::vector<uint8_t> &h, int K, int fusedN, int sign, c
                                          : (int)(((long)(TABLE_N / K) * j * k) % TABLE_N);
                     const int a[2] = {residue_of(T.c[t], m), residue_of((int64_t)sign * T.s[t], m)};
                     for (int half = 0; half < 2; half++) {
-                        const int av = a[half], ap = (av * 128) % m;  // a and a' = 128 a mod m
+                        const int av = a[half], ap = (av * 256) % m;  // a and a' = 256 a mod m
                         for (int d = 0; d < 2; d++) {                 // digit plane -> output row 2k + d
                             const int n = 2 * k + d;
-                            const int e0 = d ? av >> 7 : av & 127, e1 = d ? ap >> 7 : ap & 127;
+                            const int e0 = d ? av >> 8 : av & 255, e1 = d ? ap >> 8 : ap & 255;
                             const int kap = half * 2 * KP + 2 * j;  // byte index in the contraction
                             dst[(kap / 16) * (2 * KP * 16) + n * 16 + kap % 16] = (uint8_t)e0;
                             dst[((kap + 1) / 16) * (2 * KP * 16) + n * 16 + (kap + 1) % 16] = (uint8_t)e1;
@@ -57,9 +62,6 @@ inline void build_mat_tc(std::vector<uint8_t> &h, int K, int fusedN, int sign, c
                 }
         }
 }
-
-// -x per packed byte for bytes in [0, 127] (digits are non-negative), no carries between bytes
-__device__ __forceinline__ uint32_t neg_bytes(uint32_t x) { return ((x ^ 0x7F7F7F7Fu) + 0x01010101u) ^ 0x80808080u; }
 
 template <int KP>
 __global__ void __launch_bounds__(128 * tc_q(KP), KP >= 32 ? 1 : 2) stage_tc_kernel(StageGeom g, const uint64_t *__restrict__ in,
@@ -99,7 +101,7 @@ __global__ void __launch_bounds__(128 * tc_q(KP), KP >= 32 ? 1 : 2) stage_tc_ker
     __syncthreads();
     tc_fence_after();
     const uint32_t tmem = s_tmem;
-    const uint32_t idesc = make_idesc(CFMT_S32, I8_S8, I8_S8, 128, NCOL);
+    const uint32_t idesc = make_idesc(CFMT_S32, I8_U8, I8_U8, 128, NCOL);
     const uint32_t lane_taddr = tmem + ((uint32_t)((warp & 3) * 32) << 16);
     const uint32_t full_addr = smem_u32(&bar_full[0]);
 
@@ -141,7 +143,6 @@ __global__ void __launch_bounds__(128 * tc_q(KP), KP >= 32 ? 1 : 2) stage_tc_ker
     int tpar = 0;
     uint32_t pa_phase = 0;  // parity of the next completion of each Phase-A barrier
     uint32_t full_ph = 0, load_ph = 0;  // same for the MMA-done and matrix-landed barriers (bit = buffer)
-    const uint32_t nm7 = part ? 0x7F7F7F7Fu : 0u, nm1 = part ? 0x01010101u : 0u, nm8 = part ? 0x80808080u : 0u;
 
 #pragma unroll 1
     for (; tile < ntiles; tile += gridDim.x, tpar ^= 1) {
@@ -199,13 +200,11 @@ __global__ void __launch_bounds__(128 * tc_q(KP), KP >= 32 ? 1 : 2) stage_tc_ker
         else { tmem_ld_x4(ta, r0); tmem_ld_x4(ta + 64, r1); }
         tmem_ld_wait();
         const int i0 = 2 * p;
-        const uint32_t negm0 = 0u - kc.m[i0], mu0 = kc.mu[i0], off0 = kc.offtc[i0];
-        const uint32_t negm1 = 0u - kc.m[i0 + 1], mu1 = kc.mu[i0 + 1], off1 = kc.offtc[i0 + 1];
+        const uint32_t negm0 = 0u - kc.m[i0], mu0 = kc.mu[i0], negm1 = 0u - kc.m[i0 + 1], mu1 = kc.mu[i0 + 1];
         uint8_t *dst = sR + (q * JC) * 4096 + (i0 >> 3) * 2048 + row * 16 + (i0 & 7) * 2;
 #pragma unroll
         for (int kk = 0; kk < JC; kk++) {  // residues left in [0, 2m): any representative serves the CRT
-            const uint32_t v0 = (uint32_t)((int)r0[2 * kk + 1] * 128 + (int)r0[2 * kk]) + off0;
-            const uint32_t v1 = (uint32_t)((int)r1[2 * kk + 1] * 128 + (int)r1[2 * kk]) + off1;
+            const uint32_t v0 = r0[2 * kk + 1] * 256 + r0[2 * kk], v1 = r1[2 * kk + 1] * 256 + r1[2 * kk];  // < 2^26
             const uint32_t a = v0 + __umulhi(v0, mu0) * negm0, b = v1 + __umulhi(v1, mu1) * negm1;
             *(uint32_t *)(dst + kk * 4096) = a | (b << 16);
         }
@@ -227,14 +226,13 @@ __global__ void __launch_bounds__(128 * tc_q(KP), KP >= 32 ? 1 : 2) stage_tc_ker
                 uint32_t rr = x0[jj] + x1[jj] * c18 + x2[jj] * c36;  // < 2^30
                 rr += __umulhi(rr, mu) * negm;                        // in [0, 2m)
                 if ((negmask >> jj) & 1) rr = m2 - rr;                // -x: in (0, 2m]
-                const uint32_t hw = rr + (rr & 0xFF80u);              // digits x0 = rr & 127, x1 = rr >> 7 as two bytes
-                if (jj & 1) w[jj >> 1] |= hw << 16;
-                else w[jj >> 1] = hw;
+                if (jj & 1) w[jj >> 1] |= rr << 16;                   // the u16 IS the digit pair (rr & 255, rr >> 8)
+                else w[jj >> 1] = rr;
             }
             // own digits: first half of the own row; second half of the partner row (row^1), negated when this is
             // the im thread (the re row holds [x_R ; -x_I], the im row [x_I ; x_R])
 #pragma unroll
-            for (int t = 0; t < JC / 2; t++) o[t] = ((w[t] ^ nm7) + nm1) ^ nm8;
+            for (int t = 0; t < JC / 2; t++) o[t] = part ? m2 * 0x10001u - w[t] : w[t];  // per half-word 2m - r, no borrow
             uint8_t *A = sA + h2 * ABYTES;
             const int kap = q * JC * 2;  // first contraction byte of this thread within a half
             uint8_t *d0 = A + (kap >> 4) * (128 * 16) + row * 16 + (kap & 15);
