@@ -61,6 +61,20 @@ __device__ __forceinline__ uint64_t quantise_mag(uint64_t b, int Tmax) {
     return q;
 }
 
+// same value as quantise_mag; normal numbers (the usual case) take a short branch-free path:
+// q = mant >> sh, the dropped bits left-aligned give the guard bit and the sticky flag
+__device__ __forceinline__ uint64_t quantise_mag_fast(uint64_t b, int Tmax) {
+    const int ef = (int)((b >> 52) & 0x7FF);
+    if (ef == 0) return quantise_mag(b, Tmax);  // zero or subnormal
+    const uint64_t mant = (b & 0xFFFFFFFFFFFFFull) | (1ull << 52);
+    const int sh = Tmax + 1023 - ef;  // >= 0 because Tmax is the column maximum
+    if (sh == 0) return mant;
+    if (sh > 54) return 0;            // below half a unit
+    const uint64_t q = mant >> sh, dropped = mant << (64 - sh);
+    const uint64_t up = (dropped >> 63) & ((uint64_t)((dropped << 1) != 0) | q);
+    return q + (up & 1);
+}
+
 // r in [0, 2^32) -> r mod m by Barrett with mu = floor(2^32/m): one multiply-high, one conditional subtract
 __device__ __forceinline__ uint32_t barrett(uint32_t r, uint32_t m, uint32_t mu) {
     uint32_t q = __umulhi(r, mu);

@@ -22,6 +22,13 @@ struct StageGeom {
     int order;           // enumeration order of a launch: 0 -> b fastest, 1 -> s fastest (then b), o slowest
 };
 
+// the same with nbt = 2^lg_nbt and ns = 2^lg_ns (every supported size is a power of two): shifts, no division
+__device__ __forceinline__ void tile_coords_pow2(const StageGeom &g, long long t, int lg_nbt, int lg_ns, int &b, int &s, int &o) {
+    const uint32_t u = (uint32_t)t;
+    if (g.order == 0) { b = u & ((1u << lg_nbt) - 1); s = (u >> lg_nbt) & ((1u << lg_ns) - 1); o = u >> (lg_nbt + lg_ns); }
+    else { s = u & ((1u << lg_ns) - 1); b = (u >> lg_ns) & ((1u << lg_nbt) - 1); o = u >> (lg_nbt + lg_ns); }
+}
+
 // linear tile index -> (b, s, o) with nbt tiles along b
 __host__ __device__ inline void tile_coords(const StageGeom &g, long long t, int nbt, int &b, int &s, int &o) {
     if (g.order == 0) { b = (int)(t % nbt); t /= nbt; s = (int)(t % g.ns); o = (int)(t / g.ns); }

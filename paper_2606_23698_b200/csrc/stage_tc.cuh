@@ -86,7 +86,8 @@ __global__ void __launch_bounds__(128 * tc_q(KP), KP >= 32 ? 1 : 2) stage_tc_ker
     const int row = (warp & 3) * 32 + lane, q = warp >> 2;  // q < Q
     const int col = row >> 1, part = row & 1;
     const int K = g.K;
-    const int nbt = (g.nb + 1) >> 1;
+    // tile grid along b rounded up to a power of two (surplus tiles are fully masked); ns is a power of two
+    const int lg_nbt = 32 - __clz(((g.nb + 1) >> 1) - 1), lg_ns = 31 - __clz(g.ns);
 
     if (tid < 64) { s_tmax[0][tid] = s_tmax[1][tid] = -100000; s_flag[0][tid] = s_flag[1][tid] = 0; }
     if (tid < 128) ((uint32_t *)sPA)[tid] = kc.phaseA[tid];
@@ -108,7 +109,7 @@ __global__ void __launch_bounds__(128 * tc_q(KP), KP >= 32 ? 1 : 2) stage_tc_ker
     // per-tile addressing: (valid, input base, output base, matrix base)
     auto locate = [&](long long t, bool &valid, long long &ib, long long &ob, const uint8_t *&mb) {
         int tb, ts, to;
-        tile_coords(g, t, nbt, tb, ts, to);
+        tile_coords_pow2(g, t, lg_nbt, lg_ns, tb, ts, to);
         const int blk = 2 * tb + (col >> 5);
         valid = blk < g.nb;
         ib = blk * g.ib + ts * g.is + to * g.io + (col & 31) * g.lane;
@@ -167,7 +168,7 @@ __global__ void __launch_bounds__(128 * tc_q(KP), KP >= 32 ? 1 : 2) stage_tc_ker
     uint32_t negmask = 0;
 #pragma unroll
     for (int jj = 0; jj < JC; jj++) {
-        const uint64_t a = (flag == 1) ? quantise_mag(bits[jj], Tmax) : 0ull;
+        const uint64_t a = (flag == 1) ? quantise_mag_fast(bits[jj], Tmax) : 0ull;
         x0[jj] = (uint32_t)a & 0x3FFFF;
         x1[jj] = (uint32_t)(a >> 18) & 0x3FFFF;
         x2[jj] = (uint32_t)(a >> 36);
@@ -373,7 +374,11 @@ inline bool stage_tc_launch(const StageGeom &g, const void *src, void *dst, cons
         cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
     }
     const int KP = tc_pad(g.K);
-    const long long nt = (long long)((g.nb + 1) / 2) * g.ns * g.no;
+    int nbt = 1;
+    while (nbt < (g.nb + 1) / 2) nbt <<= 1;  // rounded up to a power of two: shifts instead of divisions on the device
+    if (g.ns & (g.ns - 1)) return false;
+    const long long nt = (long long)nbt * g.ns * g.no;
+    if (nt >= (1ll << 31)) return false;
     const uint64_t *in = (const uint64_t *)src;
     ulonglong2 *out = (ulonglong2 *)dst;
     if (KP == 32) return stage_tc_launch_kp<32>(g, in, out, mat, nt, sms, st);
