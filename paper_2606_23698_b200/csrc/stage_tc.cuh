@@ -183,22 +183,27 @@ __global__ void __launch_bounds__(128 * tc_q(KP), KP >= 32 ? 1 : 2) stage_tc_ker
     if (more) locate(ntile, nvalid, nib, nob, nmat);
     load_inputs(more && nvalid, nib, bits);
 
-    // Moduli go through the pipeline in pairs (one barrier, one fence and one commit per pair).
-    auto epilogue = [&](int p) {  // a5: recombine digits, reduce, park the residues of moduli 2p and 2p+1
+    // Moduli go through the pipeline in pairs (one barrier, one fence and one commit per pair).  While the MMAs
+    // of pair p run, the threads reduce the accumulators of pair p-1 AND compute the digits of pair p+1 in one
+    // basic block, so two independent instruction streams fill the issue slots.
+    uint32_t r0[2 * JC], r1[2 * JC];  // accumulators of a pair as read from TMEM
+    uint32_t w[2][JC / 2], o[2][JC / 2];  // digit words of a pair: own row, partner row
+    auto acc_load = [&](int p) {  // wait for the MMAs of pair p, start reading their accumulators
         const int buf = p & 1;
         mbar_wait_addr(full_addr + 8 * buf, (full_ph >> buf) & 1);
         full_ph ^= 1u << buf;
         tc_fence_after();
-        if (tid == 0 && (p + 2 < 6 || more)) {  // MMAs of pair p are complete: their matrix buffer takes pair p+2
-            const uint8_t *src = p + 2 < 6 ? matbase + (size_t)(p + 2) * 2 * MB : nmat + (size_t)(p - 4) * 2 * MB;  // or the next tile's
+        if (tid == 0 && (p + 2 < 6 || more)) {  // their matrix buffer takes pair p+2 (or the next tile's pair p-4)
+            const uint8_t *src = p + 2 < 6 ? matbase + (size_t)(p + 2) * 2 * MB : nmat + (size_t)(p - 4) * 2 * MB;
             mbar_expect_tx(&bar_load[buf], 2 * MB);
             bulk_g2s(sB + buf * 2 * MB, src, 2 * MB, &bar_load[buf]);
         }
-        uint32_t r0[2 * JC], r1[2 * JC];
         const uint32_t ta = lane_taddr + buf * 128 + 2 * q * JC;
         if constexpr (JC == 8) { tmem_ld_x16(ta, r0); tmem_ld_x16(ta + 64, r1); }
         else if constexpr (JC == 4) { tmem_ld_x8(ta, r0); tmem_ld_x8(ta + 64, r1); }
         else { tmem_ld_x4(ta, r0); tmem_ld_x4(ta + 64, r1); }
+    };
+    auto acc_reduce = [&](int p) {  // a5: recombine digits, reduce, park the residues of moduli 2p and 2p+1
         tmem_ld_wait();
         const int i0 = 2 * p;
         const uint32_t negm0 = 0u - kc.m[i0], mu0 = kc.mu[i0], negm1 = 0u - kc.m[i0 + 1], mu1 = kc.mu[i0 + 1];
@@ -211,41 +216,39 @@ __global__ void __launch_bounds__(128 * tc_q(KP), KP >= 32 ? 1 : 2) stage_tc_ker
         }
         tc_fence_before();
     };
-
-#pragma unroll 1
-    for (int p = 0; p < 6; p++) {
-        // the data operand is single-buffered: the MMAs of pair p-1 (issued before the previous epilogue) must be done
-        if (p > 0) mbar_wait_addr(full_addr + 8 * ((p - 1) & 1), (full_ph >> ((p - 1) & 1)) & 1);
+    auto digits = [&](int p) {  // a3 (second half): residues mod m_i of own elements; the u16 is the digit pair
 #pragma unroll
         for (int h2 = 0; h2 < 2; h2++) {
-            // ---- a3 (second half): residues mod m_i of own elements -> digit bytes (x0, x1) per element
             const int i = 2 * p + h2;
             const uint32_t mu = kc.mu[i], negm = 0u - kc.m[i], m2 = kc.m2[i], c18 = kc.c18[i], c36 = kc.c36[i];
-            uint32_t w[JC / 2], o[JC / 2];
 #pragma unroll
             for (int jj = 0; jj < JC; jj++) {
                 uint32_t rr = x0[jj] + x1[jj] * c18 + x2[jj] * c36;  // < 2^30
                 rr += __umulhi(rr, mu) * negm;                        // in [0, 2m)
                 if ((negmask >> jj) & 1) rr = m2 - rr;                // -x: in (0, 2m]
-                if (jj & 1) w[jj >> 1] |= rr << 16;                   // the u16 IS the digit pair (rr & 255, rr >> 8)
-                else w[jj >> 1] = rr;
+                if (jj & 1) w[h2][jj >> 1] |= rr << 16;
+                else w[h2][jj >> 1] = rr;
             }
-            // own digits: first half of the own row; second half of the partner row (row^1), negated when this is
-            // the im thread (the re row holds [x_R ; -x_I], the im row [x_I ; x_R])
+            // partner row (row^1) gets the same digits, negated (2m - r per half-word) when this is the im thread:
+            // the re row holds [x_R ; -x_I], the im row [x_I ; x_R]
 #pragma unroll
-            for (int t = 0; t < JC / 2; t++) o[t] = part ? m2 * 0x10001u - w[t] : w[t];  // per half-word 2m - r, no borrow
+            for (int t = 0; t < JC / 2; t++) o[h2][t] = part ? m2 * 0x10001u - w[h2][t] : w[h2][t];
+        }
+    };
+    auto stage_issue = [&](int p) {  // digits -> data operand; a4: residue DFTs of moduli 2p, 2p+1 on the tensor core
+#pragma unroll
+        for (int h2 = 0; h2 < 2; h2++) {
             uint8_t *A = sA + h2 * ABYTES;
             const int kap = q * JC * 2;  // first contraction byte of this thread within a half
             uint8_t *d0 = A + (kap >> 4) * (128 * 16) + row * 16 + (kap & 15);
             uint8_t *d1 = A + ((2 * KP + kap) >> 4) * (128 * 16) + (row ^ 1) * 16 + (kap & 15);
-            if constexpr (JC == 8) { *(uint4 *)d0 = make_uint4(w[0], w[1], w[2], w[3]); *(uint4 *)d1 = make_uint4(o[0], o[1], o[2], o[3]); }
-            else if constexpr (JC == 4) { *(uint2 *)d0 = make_uint2(w[0], w[1]); *(uint2 *)d1 = make_uint2(o[0], o[1]); }
-            else { *(uint32_t *)d0 = w[0]; *(uint32_t *)d1 = o[0]; }
+            if constexpr (JC == 8) { *(uint4 *)d0 = make_uint4(w[h2][0], w[h2][1], w[h2][2], w[h2][3]); *(uint4 *)d1 = make_uint4(o[h2][0], o[h2][1], o[h2][2], o[h2][3]); }
+            else if constexpr (JC == 4) { *(uint2 *)d0 = make_uint2(w[h2][0], w[h2][1]); *(uint2 *)d1 = make_uint2(o[h2][0], o[h2][1]); }
+            else { *(uint32_t *)d0 = w[h2][0]; *(uint32_t *)d1 = o[h2][0]; }
         }
         fence_async_smem();
         tc_fence_before();
         __syncthreads();
-        // ---- a4: residue DFTs of moduli 2p, 2p+1 on the tensor core
         if (tid == 0) {
             tc_fence_after();
             mbar_wait(&bar_load[p & 1], (load_ph >> (p & 1)) & 1);
@@ -262,9 +265,28 @@ __global__ void __launch_bounds__(128 * tc_q(KP), KP >= 32 ? 1 : 2) stage_tc_ker
             }
             tc_commit(&bar_full[p & 1]);
         }
-        if (p > 0) epilogue(p - 1);
+    };
+    // the data operand is single-buffered: the MMAs of pair p must be done before pair p+1 overwrites it
+    auto operand_free = [&](int p) { mbar_wait_addr(full_addr + 8 * (p & 1), (full_ph >> (p & 1)) & 1); };
+
+    digits(0);
+    stage_issue(0);
+    digits(1);
+    operand_free(0);
+    stage_issue(1);
+#pragma unroll 1
+    for (int p = 1; p < 5; p++) {  // MMAs of pair p in flight
+        acc_load(p - 1);
+        digits(p + 1);
+        acc_reduce(p - 1);
+        operand_free(p);
+        stage_issue(p + 1);
     }
-    epilogue(5);
+    acc_load(4);
+    acc_reduce(4);
+    acc_load(5);
+    acc_reduce(5);
+
 
     // ---- a6: Phase A on the tensor core (Eq. 20, two-limb form 759-764): for each output k,
     // P[row][s] = sum over the 24 residue-limb bytes of the row x the slice matrix; u8 x u8 -> s32, N = 16.
