@@ -25,6 +25,7 @@ struct DevConsts {
     uint32_t c36[12];    // 2^36 mod m
     uint32_t m2[12];     // 2 m
     uint32_t zC;         // round(2^149 / M): zhat = (umulhi(E >> 104, zC) + 2^12) >> 13
+    uint32_t off30[12];  // smallest multiple of m >= 2^30: makes the signed plane sum of the deconstruction positive
     uint32_t phaseA[128];  // Phase-A constant matrix: 16 slice rows x 32 bytes in MMA operand order
 };
 
@@ -80,6 +81,14 @@ __device__ __forceinline__ uint32_t barrett(uint32_t r, uint32_t m, uint32_t mu)
     uint32_t q = __umulhi(r, mu);
     r -= q * m;  // in [0, 2m)
     return r >= m ? r - m : r;
+}
+
+// r < 2^32 -> a representative of r mod m in [0, 2m): q = mulhi(r, floor(2^32/m)), r + q * (-m); two instructions
+// (inline PTX so the compiler keeps the multiply-add form with the negated modulus as an operand)
+__device__ __forceinline__ uint32_t barrett_lazy(uint32_t r, uint32_t mu, uint32_t negm) {
+    uint32_t o;
+    asm("{\n\t.reg .u32 q;\n\tmul.hi.u32 q, %1, %2;\n\tmad.lo.u32 %0, q, %3, %1;\n\t}" : "=r"(o) : "r"(r), "r"(mu), "r"(negm));
+    return o;
 }
 
 // canonical residue of a 53-bit magnitude (PAPER.md:190 with 16-bit planes: sum_k limb_k * (2^16k mod m))

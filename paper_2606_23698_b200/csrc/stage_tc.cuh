@@ -24,8 +24,11 @@
 
 namespace oz {
 
+#ifndef TC_Q32
+#define TC_Q32 4
+#endif
 // threads per CTA = 128 * Q: Q thread groups share each MMA row and split its contraction elements / outputs
-__host__ __device__ constexpr int tc_q(int) { return 4; }
+__host__ __device__ constexpr int tc_q(int KP) { return KP >= 32 ? TC_Q32 : 4; }
 constexpr int TC_TMEM_COLS = 256;  // [0,128): stage accumulators (2 x 64); Phase-A sums alternate [128,256) / [0,128)
 
 // bytes of one modulus' matrix planes for padded length KP: rows n = 2k + d (d = digit 0/1), 4 KP bytes each,
@@ -71,7 +74,8 @@ __global__ void __launch_bounds__(128 * tc_q(KP), KP >= 32 ? 1 : 2) stage_tc_ker
     constexpr int JC = KP / Q;         // contraction elements (and outputs) per thread
     constexpr int ABYTES = 128 * 4 * KP;
     constexpr int MB = tc_mat_bytes(KP);
-    constexpr int NB = JC / 2;         // Phase-A batches: 2 outputs per thread = 8 MMAs of N = 16 each
+    constexpr int EPB = 8 / Q;         // outputs per thread per Phase-A batch: a batch is 8 MMAs of N = 16 (128 columns)
+    constexpr int NB = JC / EPB;       // Phase-A batches
     constexpr int NCOL = 2 * KP;       // accumulator columns per modulus
     extern __shared__ __align__(128) uint8_t smem[];
     __shared__ __align__(8) uint64_t bar_full[2], bar_load[2], bar_pa[2];
@@ -164,15 +168,14 @@ __global__ void __launch_bounds__(128 * tc_q(KP), KP >= 32 ? 1 : 2) stage_tc_ker
     const int Tmax = s_tmax[tpar][col], flag = s_flag[tpar][col];
     if (tid < 64) { s_tmax[tpar ^ 1][tid] = -100000; s_flag[tpar ^ 1][tid] = 0; }  // for the next tile
     // ---- a3 (first half): quantise to 53-bit magnitudes, keep as 18/18/17-bit limbs (PAPER.md:190 planes)
-    uint32_t x0[JC], x1[JC], x2[JC];
-    uint32_t negmask = 0;
+    uint32_t x0[JC], x1[JC], x2[JC];  // two's-complement limbs of the SIGNED x~: sum_k limb_k 2^(18k) = x~
 #pragma unroll
     for (int jj = 0; jj < JC; jj++) {
         const uint64_t a = (flag == 1) ? quantise_mag_fast(bits[jj], Tmax) : 0ull;
-        x0[jj] = (uint32_t)a & 0x3FFFF;
-        x1[jj] = (uint32_t)(a >> 18) & 0x3FFFF;
-        x2[jj] = (uint32_t)(a >> 36);
-        if (bits[jj] >> 63) negmask |= 1u << jj;
+        const uint32_t sg = (uint32_t)((int32_t)(bits[jj] >> 32) >> 31);  // all ones for a negative element
+        x0[jj] = ((((uint32_t)a & 0x3FFFF) ^ sg) - sg);
+        x1[jj] = ((((uint32_t)(a >> 18) & 0x3FFFF) ^ sg) - sg);
+        x2[jj] = (((uint32_t)(a >> 36) ^ sg) - sg);
     }
     // ---- prefetch the next tile's inputs; they are consumed at the top of the next iteration
     const long long ntile = tile + gridDim.x;
@@ -211,8 +214,7 @@ __global__ void __launch_bounds__(128 * tc_q(KP), KP >= 32 ? 1 : 2) stage_tc_ker
 #pragma unroll
         for (int kk = 0; kk < JC; kk++) {  // residues left in [0, 2m): any representative serves the CRT
             const uint32_t v0 = r0[2 * kk + 1] * 256 + r0[2 * kk], v1 = r1[2 * kk + 1] * 256 + r1[2 * kk];  // < 2^26
-            const uint32_t a = v0 + __umulhi(v0, mu0) * negm0, b = v1 + __umulhi(v1, mu1) * negm1;
-            *(uint32_t *)(dst + kk * 4096) = a | (b << 16);
+            *(uint32_t *)(dst + kk * 4096) = barrett_lazy(v0, mu0, negm0) + (barrett_lazy(v1, mu1, negm1) << 16);
         }
         tc_fence_before();
     };
@@ -220,13 +222,12 @@ __global__ void __launch_bounds__(128 * tc_q(KP), KP >= 32 ? 1 : 2) stage_tc_ker
 #pragma unroll
         for (int h2 = 0; h2 < 2; h2++) {
             const int i = 2 * p + h2;
-            const uint32_t mu = kc.mu[i], negm = 0u - kc.m[i], m2 = kc.m2[i], c18 = kc.c18[i], c36 = kc.c36[i];
+            const uint32_t mu = kc.mu[i], negm = 0u - kc.m[i], m2 = kc.m2[i], c18 = kc.c18[i], c36 = kc.c36[i], off = kc.off30[i];
 #pragma unroll
             for (int jj = 0; jj < JC; jj++) {
-                uint32_t rr = x0[jj] + x1[jj] * c18 + x2[jj] * c36;  // < 2^30
-                rr += __umulhi(rr, mu) * negm;                        // in [0, 2m)
-                if ((negmask >> jj) & 1) rr = m2 - rr;                // -x: in (0, 2m]
-                if (jj & 1) w[h2][jj >> 1] |= rr << 16;
+                // signed plane sum made positive by a multiple of m: in (0, 2^31)
+                const uint32_t rr = barrett_lazy(x1[jj] * c18 + off + x2[jj] * c36 + x0[jj], mu, negm);  // in [0, 2m)
+                if (jj & 1) w[h2][jj >> 1] += rr << 16;  // disjoint bit ranges: the add is the pack
                 else w[h2][jj >> 1] = rr;
             }
             // partner row (row^1) gets the same digits, negated (2m - r per half-word) when this is the im thread:
@@ -274,8 +275,8 @@ __global__ void __launch_bounds__(128 * tc_q(KP), KP >= 32 ? 1 : 2) stage_tc_ker
     digits(1);
     operand_free(0);
     stage_issue(1);
-#pragma unroll 1
-    for (int p = 1; p < 5; p++) {  // MMAs of pair p in flight
+#pragma unroll
+    for (int p = 1; p < 5; p++) {  // MMAs of pair p in flight (unrolled: the per-modulus constants become immediates)
         acc_load(p - 1);
         digits(p + 1);
         acc_reduce(p - 1);
@@ -301,9 +302,9 @@ __global__ void __launch_bounds__(128 * tc_q(KP), KP >= 32 ? 1 : 2) stage_tc_ker
 #pragma unroll
         for (int qq = 0; qq < Q; qq++)
 #pragma unroll
-            for (int e = 0; e < 2; e++) {
-                const int k = qq * JC + 2 * b + e;
-                mma_i8_ss(dcol + qq * 32 + e * 16, make_sdesc(smem_u32(sR) + k * 4096, 128 * 16, 128), bd, idesc_pa, 0);
+            for (int e = 0; e < EPB; e++) {
+                const int k = qq * JC + EPB * b + e;
+                mma_i8_ss(dcol + (qq * EPB + e) * 16, make_sdesc(smem_u32(sR) + k * 4096, 128 * 16, 128), bd, idesc_pa, 0);
             }
         tc_commit(&bar_pa[b & 1]);
     };
@@ -319,8 +320,9 @@ __global__ void __launch_bounds__(128 * tc_q(KP), KP >= 32 ? 1 : 2) stage_tc_ker
         mbar_wait(&bar_pa[b & 1], (pa_phase >> (b & 1)) & 1);
         pa_phase ^= 1u << (b & 1);
         tc_fence_after();
-        uint32_t P[32];
-        tmem_ld_x32(lane_taddr + ((b + 1) & 1) * 128 + q * 32, P);
+        uint32_t P[16 * EPB];
+        if constexpr (EPB == 2) tmem_ld_x32(lane_taddr + ((b + 1) & 1) * 128 + q * 32, P);
+        else tmem_ld_x16(lane_taddr + ((b + 1) & 1) * 128 + q * 16, P);
         tmem_ld_wait();
         tc_fence_before();
         __syncthreads();
@@ -329,8 +331,8 @@ __global__ void __launch_bounds__(128 * tc_q(KP), KP >= 32 ? 1 : 2) stage_tc_ker
             issue_pa(b + 2);
         }
 #pragma unroll
-        for (int e = 0; e < 2; e++) {
-            const int k = q * JC + 2 * b + e;
+        for (int e = 0; e < EPB; e++) {
+            const int k = q * JC + EPB * b + e;
             uint64_t y;
             if (flag & 2) y = 0x7FF8000000000000ull;
             else if (flag == 0) y = 0;
