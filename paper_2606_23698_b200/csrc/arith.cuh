@@ -25,6 +25,7 @@ struct DevConsts {
     uint32_t c36[12];    // 2^36 mod m
     uint32_t m2[12];     // 2 m
     uint32_t zC;         // round(2^149 / M): zhat = (umulhi(E >> 104, zC) + 2^12) >> 13
+    uint32_t m2m2[12];   // 2m in both half-words
     uint32_t off30[12];  // smallest multiple of m >= 2^30: makes the signed plane sum of the deconstruction positive
     uint32_t phaseA[128];  // Phase-A constant matrix: 16 slice rows x 32 bytes in MMA operand order
 };
@@ -90,6 +91,12 @@ __device__ __forceinline__ uint32_t barrett_lazy(uint32_t r, uint32_t mu, uint32
     asm("{\n\t.reg .u32 q;\n\tmul.hi.u32 q, %1, %2;\n\tmad.lo.u32 %0, q, %3, %1;\n\t}" : "=r"(o) : "r"(r), "r"(mu), "r"(negm));
     return o;
 }
+
+// a + b on the ALU pipe (VIADDMNMX): the integer multiplier pipe is the busier one in the stage kernel, so plain
+// adds and packs are steered away from IMAD forms
+__device__ __forceinline__ uint32_t add_alu(uint32_t a, uint32_t b) { return __viaddmax_u32(a, b, 0u); }
+// (lo & 0xFFFF) | (hi << 16) as one PRMT (ALU pipe)
+__device__ __forceinline__ uint32_t pack16(uint32_t lo, uint32_t hi) { return __byte_perm(lo, hi, 0x5410); }
 
 // canonical residue of a 53-bit magnitude (PAPER.md:190 with 16-bit planes: sum_k limb_k * (2^16k mod m))
 __device__ __forceinline__ uint32_t residue53(uint64_t a, int i, const DevConsts &c) {

@@ -83,6 +83,7 @@ void fill_consts(DevConsts &c) {
         c.c18[k] = (uint32_t)((1ull << 18) % m);
         c.c36[k] = (uint32_t)((1ull << 36) % m);
         c.m2[k] = 2 * m;
+        c.m2m2[k] = 2 * m * 0x10001u;
         c.off30[k] = (uint32_t)((((1u << 30) + m - 1) / m) * m);
     }
     {  // zC = round(2^149 / M) by binary long division

@@ -213,8 +213,8 @@ __global__ void __launch_bounds__(128 * tc_q(KP), KP >= 32 ? 1 : 2) stage_tc_ker
         uint8_t *dst = sR + (q * JC) * 4096 + (i0 >> 3) * 2048 + row * 16 + (i0 & 7) * 2;
 #pragma unroll
         for (int kk = 0; kk < JC; kk++) {  // residues left in [0, 2m): any representative serves the CRT
-            const uint32_t v0 = r0[2 * kk + 1] * 256 + r0[2 * kk], v1 = r1[2 * kk + 1] * 256 + r1[2 * kk];  // < 2^26
-            *(uint32_t *)(dst + kk * 4096) = barrett_lazy(v0, mu0, negm0) + (barrett_lazy(v1, mu1, negm1) << 16);
+            const uint32_t v0 = add_alu(r0[2 * kk + 1] << 8, r0[2 * kk]), v1 = add_alu(r1[2 * kk + 1] << 8, r1[2 * kk]);  // < 2^26
+            *(uint32_t *)(dst + kk * 4096) = pack16(barrett_lazy(v0, mu0, negm0), barrett_lazy(v1, mu1, negm1));
         }
         tc_fence_before();
     };
@@ -222,18 +222,18 @@ __global__ void __launch_bounds__(128 * tc_q(KP), KP >= 32 ? 1 : 2) stage_tc_ker
 #pragma unroll
         for (int h2 = 0; h2 < 2; h2++) {
             const int i = 2 * p + h2;
-            const uint32_t mu = kc.mu[i], negm = 0u - kc.m[i], m2 = kc.m2[i], c18 = kc.c18[i], c36 = kc.c36[i], off = kc.off30[i];
+            const uint32_t mu = kc.mu[i], negm = 0u - kc.m[i], m2m2 = kc.m2m2[i], c18 = kc.c18[i], c36 = kc.c36[i], off = kc.off30[i];
 #pragma unroll
             for (int jj = 0; jj < JC; jj++) {
                 // signed plane sum made positive by a multiple of m: in (0, 2^31)
-                const uint32_t rr = barrett_lazy(x1[jj] * c18 + off + x2[jj] * c36 + x0[jj], mu, negm);  // in [0, 2m)
-                if (jj & 1) w[h2][jj >> 1] += rr << 16;  // disjoint bit ranges: the add is the pack
+                const uint32_t rr = barrett_lazy(add_alu(x2[jj] * c36 + (x1[jj] * c18 + off), x0[jj]), mu, negm);  // in [0, 2m)
+                if (jj & 1) w[h2][jj >> 1] = pack16(w[h2][jj >> 1], rr);
                 else w[h2][jj >> 1] = rr;
             }
             // partner row (row^1) gets the same digits, negated (2m - r per half-word) when this is the im thread:
             // the re row holds [x_R ; -x_I], the im row [x_I ; x_R]
 #pragma unroll
-            for (int t = 0; t < JC / 2; t++) o[h2][t] = part ? m2 * 0x10001u - w[h2][t] : w[h2][t];
+            for (int t = 0; t < JC / 2; t++) o[h2][t] = part ? m2m2 - w[h2][t] : w[h2][t];
         }
     };
     auto stage_issue = [&](int p) {  // digits -> data operand; a4: residue DFTs of moduli 2p, 2p+1 on the tensor core
