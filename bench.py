@@ -98,8 +98,8 @@ def max_over_ranks(values, device="cpu"):
 
 
 # DRAM bytes of one stage launch at 1024^3 from the committed ncu capture (profiles/r1_final.md):
-# dram__bytes_read.sum + dram__bytes_write.sum = 17.20 + 17.14 GB against 34.36 GB algorithmic
-NCU_TRAFFIC_PER_LAUNCH = {1024: 3.434e10}
+# dram__bytes_read.sum + dram__bytes_write.sum = 17.19 + 17.14 GB against 34.36 GB algorithmic
+NCU_TRAFFIC_PER_LAUNCH = {1024: 3.4334e10}
 
 
 def cpu_oracle_sample(size, pencils):
