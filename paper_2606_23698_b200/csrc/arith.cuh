@@ -71,6 +71,12 @@ __device__ __forceinline__ uint64_t quantise_mag_fast(uint64_t b, int Tmax) {
     const uint64_t mant = (b & 0xFFFFFFFFFFFFFull) | (1ull << 52);
     const int sh = Tmax + 1023 - ef;  // >= 0 because Tmax is the column maximum
     if (sh == 0) return mant;
+    if (sh < 32) {  // elements within 2^32 of the column maximum: the dropped bits come from the low word only
+        const uint32_t lo = (uint32_t)mant, hi = (uint32_t)(mant >> 32);
+        const uint32_t qlo = __funnelshift_r(lo, hi, sh), qhi = hi >> sh, dropped = lo << (32 - sh);
+        const uint32_t up = (dropped >> 31) & ((uint32_t)((dropped << 1) != 0) | qlo);
+        return (((uint64_t)qhi << 32) | qlo) + up;  // qlo + 1 cannot carry: q < 2^53 means qhi:qlo + 1 fits
+    }
     if (sh > 54) return 0;            // below half a unit
     const uint64_t q = mant >> sh, dropped = mant << (64 - sh);
     const uint64_t up = (dropped >> 63) & ((uint64_t)((dropped << 1) != 0) | q);
@@ -244,15 +250,20 @@ __device__ __forceinline__ uint64_t pack_limbs(const uint32_t *r, int g) {
     uint32_t av[4];
     abs128(av, r, sm);
     uint32_t a0 = av[0], a1 = av[1], a2 = av[2], a3 = av[3];
-    const uint64_t hi = ((uint64_t)a3 << 32) | a2, lo = ((uint64_t)a1 << 32) | a0;
-    const int s = hi ? __clzll((long long)hi) : 64 + __clzll((long long)lo);  // left shift that puts the top bit at 127
+    int s;
+    if (a3) {  // the usual case in a transform: |R| >= 2^96
+        s = __clz((int)a3);
+    } else {
+        const uint64_t hi = a2, lo = ((uint64_t)a1 << 32) | a0;
+        s = hi ? 32 + __clz((int)a2) : 64 + __clzll((long long)lo);  // 128 for R = 0
+        if (s & 64) { a3 = a1; a2 = a0; a1 = 0; a0 = 0; }
+        if (s & 32) { a3 = a2; a2 = a1; a1 = a0; a0 = 0; }
+    }
     const int X = 127 - s - g;
-    if (X < -1022 || X > 1023 || s >= 128) {
+    if ((uint32_t)(X + 1022) > 2045u || s >= 128) {  // zero, subnormal or overflowing result: generic path
         const i128 R = (i128)(((u128)r[3] << 96) | ((u128)r[2] << 64) | ((u128)r[1] << 32) | r[0]);
         return pack_rne(R, g);
     }
-    if (s & 64) { a3 = a1; a2 = a0; a1 = 0; a0 = 0; }
-    if (s & 32) { a3 = a2; a2 = a1; a1 = a0; a0 = 0; }
     const int bs = s & 31;
     const uint32_t m3 = __funnelshift_l(a2, a3, bs), m2 = __funnelshift_l(a1, a2, bs), m1 = __funnelshift_l(a0, a1, bs), m0 = a0 << bs;
     // top 53 bits = m3 : m2[31:11]; round bit m2[10]; sticky = rest
@@ -260,8 +271,9 @@ __device__ __forceinline__ uint64_t pack_limbs(const uint32_t *r, int g) {
     const uint32_t sticky = ((m2 & 0x3FF) | m1 | m0) != 0;
     const uint32_t inc = (m2 >> 10) & (sticky | qlo) & 1;
     // exponent field X+1023 enters as (X+1022) << 52 plus the hidden bit; a mantissa carry bumps it by itself
-    uint64_t bits = ((uint64_t)(uint32_t)(X + 1022) << 52) + (((uint64_t)qhi << 32) | qlo) + inc;
-    return bits | ((uint64_t)(sm & 0x80000000u) << 32);
+    const uint32_t lo32 = qlo + inc;
+    const uint32_t hi32 = qhi + ((uint32_t)(X + 1022) << 20) + (lo32 < inc) + (sm & 0x80000000u);
+    return ((uint64_t)hi32 << 32) | lo32;
 }
 
 }  // namespace oz

@@ -151,15 +151,21 @@ __global__ void __launch_bounds__(128 * tc_q(KP), KP >= 32 ? 1 : 2) stage_tc_ker
 
 #pragma unroll 1
     for (; tile < ntiles; tile += gridDim.x, tpar ^= 1) {
-    // ---- a2: column exponent
+    // ---- a2: column exponent = max of the 11-bit exponent fields (integer compare, no fp); subnormals can
+    // only matter when the thread saw no normal number at all
     {
         int tm = -100000, fl = 0;
+        uint32_t efmax = 0;
 #pragma unroll
-        for (int jj = 0; jj < JC; jj++) {
-            int T;
-            const int cls = classify_top(bits[jj], T);
-            if (cls == CLS_FINITE) { fl |= 1; tm = max(tm, T); }
-            if (cls == CLS_NONFINITE) fl |= 2;
+        for (int jj = 0; jj < JC; jj++) efmax = max(efmax, ((uint32_t)(bits[jj] >> 32) >> 20) & 0x7FFu);
+        if (efmax == 0x7FF) fl = 2;
+        else if (efmax) { fl = 1; tm = (int)efmax - 1023; }
+        else {
+#pragma unroll
+            for (int jj = 0; jj < JC; jj++) {
+                int T;
+                if (classify_top(bits[jj], T) == CLS_FINITE) { fl = 1; tm = max(tm, T); }
+            }
         }
         if (fl & 1) atomicMax(&s_tmax[tpar][col], tm);
         if (fl) atomicOr(&s_flag[tpar][col], fl);
@@ -168,14 +174,15 @@ __global__ void __launch_bounds__(128 * tc_q(KP), KP >= 32 ? 1 : 2) stage_tc_ker
     const int Tmax = s_tmax[tpar][col], flag = s_flag[tpar][col];
     if (tid < 64) { s_tmax[tpar ^ 1][tid] = -100000; s_flag[tpar ^ 1][tid] = 0; }  // for the next tile
     // ---- a3 (first half): quantise to 53-bit magnitudes, keep as 18/18/17-bit limbs (PAPER.md:190 planes)
-    uint32_t x0[JC], x1[JC], x2[JC];  // two's-complement limbs of the SIGNED x~: sum_k limb_k 2^(18k) = x~
+    uint32_t x0[JC], x1[JC], x2[JC];  // planes of the SIGNED x~ (two unsigned, the top one signed)
 #pragma unroll
     for (int jj = 0; jj < JC; jj++) {
         const uint64_t a = (flag == 1) ? quantise_mag_fast(bits[jj], Tmax) : 0ull;
-        const uint32_t sg = (uint32_t)((int32_t)(bits[jj] >> 32) >> 31);  // all ones for a negative element
-        x0[jj] = ((((uint32_t)a & 0x3FFFF) ^ sg) - sg);
-        x1[jj] = ((((uint32_t)(a >> 18) & 0x3FFFF) ^ sg) - sg);
-        x2[jj] = (((uint32_t)(a >> 36) ^ sg) - sg);
+        const uint64_t sg = (uint64_t)((int64_t)bits[jj] >> 63);  // all ones for a negative element
+        const uint64_t v = (a ^ sg) - sg;                          // x~ in two's complement
+        x0[jj] = (uint32_t)v & 0x3FFFF;                            // unsigned 18 bits
+        x1[jj] = (uint32_t)(v >> 18) & 0x3FFFF;                    // unsigned 18 bits
+        x2[jj] = (uint32_t)((int32_t)(v >> 32) >> 4);              // signed top: x~ = x0 + 2^18 x1 + 2^36 x2
     }
     // ---- prefetch the next tile's inputs; they are consumed at the top of the next iteration
     const long long ntile = tile + gridDim.x;
