@@ -54,11 +54,16 @@ struct ozfft_plan_s {
     DevConsts *d_consts;
     void *work;
     void *h_in, *h_out;  // device staging for ozfft_exec_host (lazy)
+    bool pipelined;      // exec_host overlaps the copies with the passes
+    std::vector<StageLaunch> slab_stages;  // z and y stages of one slab of nx/PIPE planes
+    cudaStream_t s_in, s_out;
+    cudaEvent_t ev_in[8], ev_out[8], ev_start;
 };
 
 namespace {
 
 constexpr uint32_t PLAN_MAGIC = 0x4F5A4646u;
+constexpr int PIPE = 8;  // slabs / chunks of the host-buffer pipeline
 
 bool is_pow2(int n) { return n >= 2 && (n & (n - 1)) == 0; }
 
@@ -158,7 +163,8 @@ struct AxisDesc {
     long long outer, N, inner;  // strided: element (o, i, z) at (o*N + i)*inner + z; contiguous: pencil P at P*N
 };
 
-bool add_axis(ozfft_plan_s *p, const AxisDesc &a, int axis, std::map<MatKey, std::pair<const ushort2 *, const uint8_t *>> &mats) {
+bool add_axis(ozfft_plan_s *p, const AxisDesc &a, int axis, std::map<MatKey, std::pair<const ushort2 *, const uint8_t *>> &mats,
+              std::vector<StageLaunch> &dst) {
     const int N = (int)a.N;
     const bool two = N > 32;
     const int q = two ? 32 : N, pp = two ? N / 32 : 1;
@@ -209,10 +215,10 @@ bool add_axis(ozfft_plan_s *p, const AxisDesc &a, int axis, std::map<MatKey, std
     }
     g1.ob = g1.ib; g1.os = g1.is; g1.oo = g1.io;
     if (!get(q, 0, s1)) return false;
-    p->stages.push_back(s1);
+    dst.push_back(s1);
     if (two) {
         if (!get(pp, N, s2)) return false;
-        p->stages.push_back(s2);
+        dst.push_back(s2);
     }
     return true;
 }
@@ -237,17 +243,27 @@ ozfft_plan_s *make_plan(int nx, int ny, int nz, int sign, bool batched1d) {
     p->variant = pick_variant();
     p->dev_bytes = 0;
     p->work = p->h_in = p->h_out = nullptr;
+    p->pipelined = false;
+    p->s_in = p->s_out = nullptr;
     DevConsts hc;
     fill_consts(hc);
     p->d_consts = (DevConsts *)dev_upload(p, &hc, sizeof(hc));
     std::map<MatKey, std::pair<const ushort2 *, const uint8_t *>> mats;
     bool ok = p->d_consts != nullptr;
     if (batched1d) {  // nx = batch, nz = n
-        ok = ok && add_axis(p, AxisDesc{true, nx, nz, 1}, 0, mats);
+        ok = ok && add_axis(p, AxisDesc{true, nx, nz, 1}, 0, mats, p->stages);
     } else {
-        ok = ok && add_axis(p, AxisDesc{true, (long long)nx * ny, nz, 1}, 0, mats);
-        ok = ok && add_axis(p, AxisDesc{false, nx, ny, nz}, 1, mats);
-        ok = ok && add_axis(p, AxisDesc{false, 1, nx, (long long)ny * nz}, 2, mats);
+        ok = ok && add_axis(p, AxisDesc{true, (long long)nx * ny, nz, 1}, 0, mats, p->stages);
+        ok = ok && add_axis(p, AxisDesc{false, nx, ny, nz}, 1, mats, p->stages);
+        ok = ok && add_axis(p, AxisDesc{false, 1, nx, (long long)ny * nz}, 2, mats, p->stages);
+        // host-buffer pipeline (ozfft_exec_host): the z and y passes run per slab of nx/8 planes as the slabs arrive,
+        // the x pass per chunk of ny/8 rows whose results leave while the next chunk computes
+        const int xs = nx / PIPE, yc = ny / PIPE;
+        if (ok && nx >= PIPE && ny >= PIPE && p->count >= (1ll << 24) && ((long long)xs * ny) % 64 == 0 && ((long long)yc * nz) % 64 == 0) {
+            ok = ok && add_axis(p, AxisDesc{true, (long long)xs * ny, nz, 1}, 0, mats, p->slab_stages);
+            ok = ok && add_axis(p, AxisDesc{false, xs, ny, nz}, 1, mats, p->slab_stages);
+            p->pipelined = ok;
+        }
     }
     if (ok) {
         ok = cuda_ok(cudaMalloc(&p->work, (size_t)p->count * 16), "cudaMalloc(workspace)");
@@ -339,6 +355,60 @@ int ozfft_exec_axis(ozfft_plan p, int axis, const void *in, void *out, void *str
     return run_stages(p, first, last, in, out, (cudaStream_t)stream);
 }
 
+// pipelined host-buffer transform of a 3-D plan: H2D slab s || z,y passes of slab s-1;  x pass of chunk c || D2H of chunk c-1
+static int exec_host_pipelined(ozfft_plan p, const char *hin, char *hout, cudaStream_t st) {
+    const long long nx = p->nx, ny = p->ny, nz = p->nz;
+    const long long xs = nx / PIPE, yc = ny / PIPE;
+    const size_t slab_elems = (size_t)(xs * ny * nz), slab_bytes = slab_elems * 16;
+    if (!p->s_in) {
+        if (!cuda_ok(cudaStreamCreateWithFlags(&p->s_in, cudaStreamNonBlocking), "cudaStreamCreate") ||
+            !cuda_ok(cudaStreamCreateWithFlags(&p->s_out, cudaStreamNonBlocking), "cudaStreamCreate")) return OZFFT_ECUDA;
+        for (int i = 0; i < PIPE; i++) {
+            cudaEventCreateWithFlags(&p->ev_in[i], cudaEventDisableTiming);
+            cudaEventCreateWithFlags(&p->ev_out[i], cudaEventDisableTiming);
+        }
+        cudaEventCreateWithFlags(&p->ev_start, cudaEventDisableTiming);
+    }
+    const size_t L = p->stages.size(), Lzy = p->slab_stages.size();
+    auto buf_of = [&](size_t i) -> char * { return (char *)(((L - 1 - i) & 1) ? p->work : p->h_out); };  // as run_stages
+    // copies start once earlier work on the caller's stream is done
+    cudaEventRecord(p->ev_start, st);
+    cudaStreamWaitEvent(p->s_in, p->ev_start, 0);
+    cudaStreamWaitEvent(p->s_out, p->ev_start, 0);
+    for (int s = 0; s < PIPE; s++) {
+        if (!cuda_ok(cudaMemcpyAsync((char *)p->h_in + s * slab_bytes, hin + s * slab_bytes, slab_bytes, cudaMemcpyHostToDevice, p->s_in), "H2D slab")) return OZFFT_ECUDA;
+        cudaEventRecord(p->ev_in[s], p->s_in);
+    }
+    for (int s = 0; s < PIPE; s++) {  // z and y passes of slab s
+        cudaStreamWaitEvent(st, p->ev_in[s], 0);
+        const char *src = (const char *)p->h_in + s * slab_bytes;
+        for (size_t i = 0; i < Lzy; i++) {
+            char *dst = buf_of(i) + s * slab_bytes;
+            int rc = launch_stage(p, p->slab_stages[i], src, dst, st);
+            if (rc) return rc;
+            src = dst;
+        }
+    }
+    for (int c = 0; c < PIPE; c++) {  // x pass of the rows y in [c*yc, (c+1)*yc), then their way home
+        const size_t off = (size_t)(c * yc * nz) * 16;
+        const char *src = (Lzy ? buf_of(Lzy - 1) : (char *)p->h_in) + off;
+        for (size_t i = Lzy; i < L; i++) {
+            StageLaunch sl = p->stages[i];
+            sl.g.nb = (int)(yc * nz / 32);
+            char *dst = buf_of(i) + off;
+            int rc = launch_stage(p, sl, src, dst, st);
+            if (rc) return rc;
+            src = dst;
+        }
+        cudaEventRecord(p->ev_out[c], st);
+        cudaStreamWaitEvent(p->s_out, p->ev_out[c], 0);
+        if (!cuda_ok(cudaMemcpy2DAsync(hout + off, (size_t)(ny * nz) * 16, (char *)p->h_out + off, (size_t)(ny * nz) * 16,
+                                       (size_t)(yc * nz) * 16, (size_t)nx, cudaMemcpyDeviceToHost, p->s_out), "D2H chunk")) return OZFFT_ECUDA;
+    }
+    if (!cuda_ok(cudaStreamSynchronize(p->s_out), "cudaStreamSynchronize")) return OZFFT_ECUDA;
+    return cuda_ok(cudaStreamSynchronize(st), "cudaStreamSynchronize") ? OZFFT_OK : OZFFT_ECUDA;
+}
+
 int ozfft_exec_host(ozfft_plan p, const void *host_in, void *host_out, void *stream) {
     if (!valid(p)) { set_err("invalid or destroyed plan"); return OZFFT_EINVAL; }
     if (!host_in || !host_out) { set_err("null host pointer"); return OZFFT_EINVAL; }
@@ -349,6 +419,7 @@ int ozfft_exec_host(ozfft_plan p, const void *host_in, void *host_out, void *str
         p->dev_bytes += 2 * bytes;
     }
     cudaStream_t st = (cudaStream_t)stream;
+    if (p->pipelined && !getenv("OZFFT_NO_PIPELINE")) return exec_host_pipelined(p, (const char *)host_in, (char *)host_out, st);
     if (!cuda_ok(cudaMemcpyAsync(p->h_in, host_in, bytes, cudaMemcpyHostToDevice, st), "H2D")) return OZFFT_ECUDA;
     int rc = run_stages(p, 0, p->stages.size(), p->h_in, p->h_out, st);
     if (rc) return rc;
@@ -362,6 +433,12 @@ void ozfft_plan_destroy(ozfft_plan p) {
     if (p->work) cudaFree(p->work);
     if (p->h_in) cudaFree(p->h_in);
     if (p->h_out) cudaFree(p->h_out);
+    if (p->s_in) {
+        cudaStreamDestroy(p->s_in);
+        cudaStreamDestroy(p->s_out);
+        for (int i = 0; i < PIPE; i++) { cudaEventDestroy(p->ev_in[i]); cudaEventDestroy(p->ev_out[i]); }
+        cudaEventDestroy(p->ev_start);
+    }
     p->magic = 0;
     delete p;
 }

@@ -161,3 +161,24 @@ def test_bad_arguments():
     assert ozfft.lib().ozfft_exec(plan.h, x.data_ptr(), x.data_ptr(), None) == 1  # in == out
     assert ozfft.lib().ozfft_exec(plan.h, x.data_ptr() + 8, x.data_ptr(), None) == 1  # misaligned
     plan.destroy()
+
+
+def test_exec_host_pipelined_path(O, variant):
+    """sizes >= 2^24 elements take the slab pipeline in ozfft_exec_host (copies overlapped with the passes):
+    same bits as the device-resident call and as the oracle"""
+    if variant != "tc":
+        pytest.skip("pipeline logic is kernel-independent; run once")
+    torch = _torch()
+    from paper_2606_23698_b200 import inputs, ozfft
+    shape = (256, 256, 256)
+    x = inputs.uniform_pm1(shape, 21)
+    plan = ozfft.Plan(*shape)
+    xin = torch.from_numpy(x).pin_memory()
+    out = torch.empty_like(xin).pin_memory()
+    plan.exec_host(xin, out)
+    dev = plan.exec(torch.from_numpy(x).cuda()).cpu()
+    assert torch.equal(out.view(torch.float64), dev.view(torch.float64))
+    _assert_bit_exact(out.numpy(), O.fft3d(x, -1, route=0)[0])
+    plan.exec_host(xin, out)  # a second call reuses streams and events
+    assert torch.equal(out.view(torch.float64), dev.view(torch.float64))
+    plan.destroy()
