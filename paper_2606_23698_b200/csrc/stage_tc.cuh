@@ -111,20 +111,22 @@ __global__ void __launch_bounds__(128 * tc_q(KP), KP >= 32 ? 1 : 2) stage_tc_ker
     const uint32_t full_addr = smem_u32(&bar_full[0]);
 
     // per-tile addressing: (valid, input base, output base, matrix base)
-    auto locate = [&](long long t, bool &valid, long long &ib, long long &ob, const uint8_t *&mb) {
+    // element offsets fit 32 bits (at most 2^30 elements per array); they widen only when the address is formed
+    auto locate = [&](long long t, bool &valid, uint32_t &ib, uint32_t &ob, const uint8_t *&mb) {
         int tb, ts, to;
         tile_coords_pow2(g, t, lg_nbt, lg_ns, tb, ts, to);
         const int blk = 2 * tb + (col >> 5);
         valid = blk < g.nb;
-        ib = blk * g.ib + ts * g.is + to * g.io + (col & 31) * g.lane;
-        ob = blk * g.ob + ts * g.os + to * g.oo + (col & 31) * g.lane;
+        ib = (uint32_t)blk * (uint32_t)g.ib + (uint32_t)ts * (uint32_t)g.is + (uint32_t)to * (uint32_t)g.io + (uint32_t)(col & 31) * (uint32_t)g.lane;
+        ob = (uint32_t)blk * (uint32_t)g.ob + (uint32_t)ts * (uint32_t)g.os + (uint32_t)to * (uint32_t)g.oo + (uint32_t)(col & 31) * (uint32_t)g.lane;
         mb = mat + (size_t)(g.matsel ? ts : 0) * 12 * MB;
     };
-    auto load_inputs = [&](bool valid, long long ib, uint64_t *bits) {  // a1: own part of own contraction elements
+    const uint32_t ji32 = (uint32_t)g.ji, ko32 = (uint32_t)g.ko;
+    auto load_inputs = [&](bool valid, uint32_t ib, uint64_t *bits) {  // a1: own part of own contraction elements
 #pragma unroll
         for (int jj = 0; jj < JC; jj++) {
             const int j = q * JC + jj;
-            bits[jj] = (valid && j < K) ? __ldg(in + 2 * (ib + j * g.ji) + part) : 0ull;
+            bits[jj] = (valid && j < K) ? __ldg(in + 2 * (size_t)(ib + (uint32_t)j * ji32) + part) : 0ull;
         }
     };
 
@@ -134,7 +136,7 @@ __global__ void __launch_bounds__(128 * tc_q(KP), KP >= 32 ? 1 : 2) stage_tc_ker
         return;
     }
     bool colvalid;
-    long long ibase, obase;
+    uint32_t ibase, obase;
     const uint8_t *matbase;
     locate(tile, colvalid, ibase, obase, matbase);
     if (tid == 0) {  // matrix planes of modulus pairs 0 and 1 of the first tile
@@ -188,7 +190,7 @@ __global__ void __launch_bounds__(128 * tc_q(KP), KP >= 32 ? 1 : 2) stage_tc_ker
     const long long ntile = tile + gridDim.x;
     const bool more = ntile < ntiles;
     bool nvalid = false;
-    long long nib = 0, nob = 0;
+    uint32_t nib = 0, nob = 0;
     const uint8_t *nmat = matbase;
     if (more) locate(ntile, nvalid, nib, nob, nmat);
     load_inputs(more && nvalid, nib, bits);
@@ -354,7 +356,7 @@ __global__ void __launch_bounds__(128 * tc_q(KP), KP >= 32 ? 1 : 2) stage_tc_ker
                 ulonglong2 o;
                 o.x = part ? yp : y;
                 o.y = part ? y : yp;
-                out[obase + k * g.ko] = o;
+                out[(size_t)(obase + (uint32_t)k * ko32)] = o;
             }
         }
     }
