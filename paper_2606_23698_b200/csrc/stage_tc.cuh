@@ -29,7 +29,8 @@ namespace oz {
 #endif
 // threads per CTA = 128 * Q: Q thread groups share each MMA row and split its contraction elements / outputs
 __host__ __device__ constexpr int tc_q(int KP) { return KP >= 32 ? TC_Q32 : 4; }
-constexpr int TC_TMEM_COLS = 256;  // [0,128): stage accumulators (2 x 64); Phase-A sums alternate [128,256) / [0,128)
+// TMEM columns: [0,256) stage accumulators (2 pairs x 2 x 64); the Phase-A sums of batch b reuse [128 b, 128 b + 128)
+__host__ __device__ constexpr int tc_tmem_cols(int KP) { return KP >= 32 ? 512 : 256; }
 
 // bytes of one modulus' matrix planes for padded length KP: rows n = 2k + d (d = digit 0/1), 4 KP bytes each,
 // stored in the canonical K-major no-swizzle core-matrix order [chunk = byte/16][row n][16 B]
@@ -78,7 +79,7 @@ __global__ void __launch_bounds__(128 * tc_q(KP), KP >= 32 ? 1 : 2) stage_tc_ker
     constexpr int NB = JC / EPB;       // Phase-A batches
     constexpr int NCOL = 2 * KP;       // accumulator columns per modulus
     extern __shared__ __align__(128) uint8_t smem[];
-    __shared__ __align__(8) uint64_t bar_full[2], bar_load[2], bar_pa[2];
+    __shared__ __align__(8) uint64_t bar_full[2], bar_load[2], bar_pa[4];
     __shared__ uint32_t s_tmem;
     __shared__ int s_tmax[2][64], s_flag[2][64];
     uint8_t *sA = smem, *sB = smem + 2 * ABYTES, *sR = smem + 2 * ABYTES + 4 * MB;
@@ -95,11 +96,11 @@ __global__ void __launch_bounds__(128 * tc_q(KP), KP >= 32 ? 1 : 2) stage_tc_ker
 
     if (tid < 64) { s_tmax[0][tid] = s_tmax[1][tid] = -100000; s_flag[0][tid] = s_flag[1][tid] = 0; }
     if (tid < 128) ((uint32_t *)sPA)[tid] = kc.phaseA[tid];
-    if (warp == 0) tmem_alloc<TC_TMEM_COLS>(&s_tmem);
+    if (warp == 0) tmem_alloc<tc_tmem_cols(KP)>(&s_tmem);
     if (tid == 0) {
         mbar_init(&bar_full[0], 1); mbar_init(&bar_full[1], 1);
         mbar_init(&bar_load[0], 1); mbar_init(&bar_load[1], 1);
-        mbar_init(&bar_pa[0], 1); mbar_init(&bar_pa[1], 1);
+        for (int i = 0; i < 4; i++) mbar_init(&bar_pa[i], 1);
         mbar_fence_init();
     }
     tc_fence_before();
@@ -132,7 +133,7 @@ __global__ void __launch_bounds__(128 * tc_q(KP), KP >= 32 ? 1 : 2) stage_tc_ker
 
     long long tile = blockIdx.x;
     if (tile >= ntiles) {  // (never with grid <= ntiles) still release TMEM
-        if (warp == 0) tmem_dealloc<TC_TMEM_COLS>(tmem);
+        if (warp == 0) tmem_dealloc<tc_tmem_cols(KP)>(tmem);
         return;
     }
     bool colvalid;
@@ -148,7 +149,7 @@ __global__ void __launch_bounds__(128 * tc_q(KP), KP >= 32 ? 1 : 2) stage_tc_ker
     uint64_t bits[JC];
     load_inputs(colvalid, ibase, bits);
     int tpar = 0;
-    uint32_t pa_phase = 0;  // parity of the next completion of each Phase-A barrier
+    uint32_t pa_phase = 0;  // parity of the next completion of the Phase-A barriers (one completion per tile each)
     uint32_t full_ph = 0, load_ph = 0;  // same for the MMA-done and matrix-landed barriers (bit = buffer)
 
 #pragma unroll 1
@@ -307,7 +308,7 @@ __global__ void __launch_bounds__(128 * tc_q(KP), KP >= 32 ? 1 : 2) stage_tc_ker
     auto issue_pa = [&](int b) {
         const uint32_t idesc_pa = make_idesc(CFMT_S32, I8_U8, I8_U8, 128, 16);
         const uint64_t bd = make_sdesc(smem_u32(sPA), 16 * 16, 128);
-        const uint32_t dcol = tmem + ((b + 1) & 1) * 128;
+        const uint32_t dcol = tmem + b * 128;
 #pragma unroll
         for (int qq = 0; qq < Q; qq++)
 #pragma unroll
@@ -315,30 +316,23 @@ __global__ void __launch_bounds__(128 * tc_q(KP), KP >= 32 ? 1 : 2) stage_tc_ker
                 const int k = qq * JC + EPB * b + e;
                 mma_i8_ss(dcol + (qq * EPB + e) * 16, make_sdesc(smem_u32(sR) + k * 4096, 128 * 16, 128), bd, idesc_pa, 0);
             }
-        tc_commit(&bar_pa[b & 1]);
+        tc_commit(&bar_pa[b]);
     };
     if (tid == 0) {
         tc_fence_after();
-        issue_pa(0);
-        if (NB > 1) issue_pa(1);
+#pragma unroll
+        for (int b = 0; b < NB; b++) issue_pa(b);  // every batch has its own TMEM columns: no barrier between batches
     }
     // ---- a7-a9: Phase B deposits, lift, pack; a12: store (the re thread stores even k, the im thread odd k)
     const int gexp = 53 + 52 - Tmax;
 #pragma unroll 1
     for (int b = 0; b < NB; b++) {
-        mbar_wait(&bar_pa[b & 1], (pa_phase >> (b & 1)) & 1);
-        pa_phase ^= 1u << (b & 1);
+        mbar_wait(&bar_pa[b], pa_phase);
         tc_fence_after();
         uint32_t P[16 * EPB];
-        if constexpr (EPB == 2) tmem_ld_x32(lane_taddr + ((b + 1) & 1) * 128 + q * 32, P);
-        else tmem_ld_x16(lane_taddr + ((b + 1) & 1) * 128 + q * 16, P);
+        if constexpr (EPB == 2) tmem_ld_x32(lane_taddr + b * 128 + q * 32, P);
+        else tmem_ld_x16(lane_taddr + b * 128 + q * 16, P);
         tmem_ld_wait();
-        tc_fence_before();
-        __syncthreads();
-        if (tid == 0 && b + 2 < NB) {
-            tc_fence_after();
-            issue_pa(b + 2);
-        }
 #pragma unroll
         for (int e = 0; e < EPB; e++) {
             const int k = q * JC + EPB * b + e;
@@ -360,11 +354,13 @@ __global__ void __launch_bounds__(128 * tc_q(KP), KP >= 32 ? 1 : 2) stage_tc_ker
             }
         }
     }
+    pa_phase ^= 1;
+    tc_fence_before();  // the next tile's MMAs overwrite the columns just read (after its barriers)
     colvalid = nvalid; ibase = nib; obase = nob; matbase = nmat;
     }  // tile loop
     tc_fence_before();
     __syncthreads();
-    if (warp == 0) tmem_dealloc<TC_TMEM_COLS>(tmem);
+    if (warp == 0) tmem_dealloc<tc_tmem_cols(KP)>(tmem);
 }
 
 inline bool stage_tc_prepare(const DevConsts &hc) {
@@ -391,7 +387,7 @@ inline bool stage_tc_launch_kp(const StageGeom &g, const uint64_t *in, ulonglong
             per_sm = by_smem < by_regs ? by_smem : by_regs;
         }
         if (per_sm < 1) per_sm = 1;
-        if (per_sm > 2) per_sm = 2;  // 2 x 256 TMEM columns
+        if (per_sm > 512 / tc_tmem_cols(KP)) per_sm = 512 / tc_tmem_cols(KP);  // TMEM columns
     }
     const long long cap = (long long)sms * per_sm;
     const unsigned grid = (unsigned)(nt < cap ? nt : cap);
