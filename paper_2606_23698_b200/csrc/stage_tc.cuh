@@ -149,14 +149,10 @@ __global__ void __launch_bounds__(128 * tc_q(KP), KP >= 32 ? 1 : 2) stage_tc_ker
     uint64_t bits[JC];
     load_inputs(colvalid, ibase, bits);
     int tpar = 0;
-    uint32_t pa_phase = 0;  // parity of the next completion of the Phase-A barriers (one completion per tile each)
-    uint32_t full_ph = 0, load_ph = 0;  // same for the MMA-done and matrix-landed barriers (bit = buffer)
-
-#pragma unroll 1
-    for (; tile < ntiles; tile += gridDim.x, tpar ^= 1) {
-    // ---- a2: column exponent = max of the 11-bit exponent fields (integer compare, no fp); subnormals can
-    // only matter when the thread saw no normal number at all
-    {
+    // a2: column exponent = max of the 11-bit exponent fields (integer compare, no fp); subnormals can only matter
+    // when the thread saw no normal number at all.  Scanned one tile ahead (the inputs are prefetched), so the
+    // result is published by barriers the pipeline has anyway.
+    auto exponent_scan = [&](int par) {
         int tm = -100000, fl = 0;
         uint32_t efmax = 0;
 #pragma unroll
@@ -170,10 +166,16 @@ __global__ void __launch_bounds__(128 * tc_q(KP), KP >= 32 ? 1 : 2) stage_tc_ker
                 if (classify_top(bits[jj], T) == CLS_FINITE) { fl = 1; tm = max(tm, T); }
             }
         }
-        if (fl & 1) atomicMax(&s_tmax[tpar][col], tm);
-        if (fl) atomicOr(&s_flag[tpar][col], fl);
-    }
+        if (fl & 1) atomicMax(&s_tmax[par][col], tm);
+        if (fl) atomicOr(&s_flag[par][col], fl);
+    };
+    exponent_scan(0);
     __syncthreads();
+    uint32_t pa_phase = 0;  // parity of the next completion of the Phase-A barriers (one completion per tile each)
+    uint32_t full_ph = 0, load_ph = 0;  // same for the MMA-done and matrix-landed barriers (bit = buffer)
+
+#pragma unroll 1
+    for (; tile < ntiles; tile += gridDim.x, tpar ^= 1) {
     const int Tmax = s_tmax[tpar][col], flag = s_flag[tpar][col];
     if (tid < 64) { s_tmax[tpar ^ 1][tid] = -100000; s_flag[tpar ^ 1][tid] = 0; }  // for the next tile
     // ---- a3 (first half): quantise to 53-bit magnitudes, keep as 18/18/17-bit limbs (PAPER.md:190 planes)
@@ -299,6 +301,7 @@ __global__ void __launch_bounds__(128 * tc_q(KP), KP >= 32 ? 1 : 2) stage_tc_ker
     acc_reduce(5);
 
 
+    exponent_scan(tpar ^ 1);  // the next tile's columns (its inputs arrived long ago); published by the barrier below
     // ---- a6: Phase A on the tensor core (Eq. 20, two-limb form 759-764): for each output k,
     // P[row][s] = sum over the 24 residue-limb bytes of the row x the slice matrix; u8 x u8 -> s32, N = 16.
     // Batch b covers outputs k = q'*JC + 2b + e (q' < 4, e < 2): thread group q' reads its 32 columns at q'*32.
