@@ -217,8 +217,10 @@ __device__ __forceinline__ void crt_limbs(const uint32_t *v, uint32_t *r) {
 __device__ __forceinline__ void deposit_slices(const uint32_t *P, uint32_t *r) {
     uint64_t w[4];
 #pragma unroll
-    for (int j = 0; j < 4; j++)
-        w[j] = (uint64_t)P[4 * j] + ((uint64_t)P[4 * j + 1] << 8) + ((uint64_t)P[4 * j + 2] << 16) + ((uint64_t)P[4 * j + 3] << 24);
+    for (int j = 0; j < 4; j++) {  // three multiply-adds per word: 32-bit, then two 32 x 32 + 64 -> 64
+        w[j] = (uint64_t)P[4 * j + 2] * 65536u + (P[4 * j] + P[4 * j + 1] * 256u);
+        w[j] = (uint64_t)P[4 * j + 3] * 16777216u + w[j];
+    }
     const uint64_t t1 = (w[0] >> 32) + w[1], t2 = (t1 >> 32) + w[2], t3 = (t2 >> 32) + w[3];
     crt_from_E((uint32_t)w[0], (uint32_t)t1, (uint32_t)t2, (uint32_t)t3, (uint32_t)(t3 >> 32), r);
 }
