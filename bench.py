@@ -100,6 +100,8 @@ def max_over_ranks(values, device="cpu"):
 # DRAM bytes of one stage launch at 1024^3 from the committed ncu capture (profiles/r1_final.md):
 # dram__bytes_read.sum + dram__bytes_write.sum = 17.19 + 17.14 GB against 34.36 GB algorithmic
 NCU_TRAFFIC_PER_LAUNCH = {1024: 3.4334e10}
+# smsp__inst_executed.sum x 32 / n_out of the same capture (predicated-off lanes included)
+NCU_THREAD_INST_PER_OUT = 376.0
 
 
 def cpu_oracle_sample(size, pencils):
@@ -263,9 +265,12 @@ def run_ours(args):
             "e2e": {"value": world * flops(n_tot) / (e2e_ms_max * 1e-3) / 1e9, "unit": "GFLOP/s", "ms": e2e_ms_max,
                     "h2d_bytes_per_step": nbytes, "d2h_bytes_per_step": nbytes, "steps": e2e_steps},
             "gpu_launches": launches * args.steps,
-            "integer_issue": {"n_out": 2 * launches * n_tot, "peak_thread_inst_per_s": 148 * 128 * 1.965e9,
-                              "note": "the path is bound by SIMT integer issue (PAPER.md:452); measured thread "
-                                      "instructions per output-equivalent and issue-slot use are in profiles/"},
+            # what actually binds: SIMT integer issue.  achieved = n_out x the ncu-measured thread
+            # instructions per output-equivalent (profiles/r1_final.md) / step time; peak = 148 SM x 128 lanes x 1.965 GHz
+            "roofline_alu": {"bound": "alu", "achieved": 2 * launches * n_tot * NCU_THREAD_INST_PER_OUT / (ms_step * 1e-3) / 1e12,
+                             "peak": 148 * 128 * 1.965e9 / 1e12, "unit": "T thread-inst/s",
+                             "frac": 2 * launches * n_tot * NCU_THREAD_INST_PER_OUT / (ms_step * 1e-3) / (148 * 128 * 1.965e9),
+                             "n_out": 2 * launches * n_tot, "thread_inst_per_output_eq": NCU_THREAD_INST_PER_OUT},
             "context": {"cufft_z2z_ms": cufft_ms, "paper_projection_ms_B300": [63, 87], "paper_projection_ms_B200": [70, 96],
                         "paper_hbm_roof_ms": 12.9},
         }
