@@ -101,7 +101,7 @@ def max_over_ranks(values, device="cpu"):
 # dram__bytes_read.sum + dram__bytes_write.sum = 17.19 + 17.14 GB against 34.36 GB algorithmic
 NCU_TRAFFIC_PER_LAUNCH = {1024: 3.4334e10}
 # smsp__inst_executed.sum x 32 / n_out of the same capture (predicated-off lanes included)
-NCU_THREAD_INST_PER_OUT = 376.0
+NCU_THREAD_INST_PER_OUT = 372.0
 
 
 def cpu_oracle_sample(size, pencils):
