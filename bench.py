@@ -164,11 +164,32 @@ def run_ours(args):
     shape = (size, size, size)
     nbytes = 16 * n_tot
 
-    # synthetic input (configs[4] recipe), generated on the host in pinned memory, rank-specific seed offset
-    h_in = torch.empty(shape, dtype=torch.complex128).pin_memory()
-    inputs.uniform_pm1(shape, SEED + 1000 * rank, out=h_in.numpy())
-    h_out = torch.empty(shape, dtype=torch.complex128).pin_memory()
-    d_in = h_in.cuda()
+    # synthetic input (configs[4] recipe), generated on the host in pinned memory, rank-specific seed offset.
+    # N ranks on one node need N x 2 x 16 GiB of pinned host memory for the end-to-end leg: if the node does not
+    # have it, the input is streamed to the device in slabs and the e2e leg is reported as skipped (never risk the box)
+    try:
+        import psutil
+        host_ok = psutil.virtual_memory().available > world * 2 * nbytes * 1.2
+    except Exception:
+        host_ok = world == 1
+    if world > 1:  # one decision for all ranks (the end-to-end leg has barriers)
+        flag = torch.tensor([1 if host_ok else 0], device="cuda")
+        dist.all_reduce(flag, op=dist.ReduceOp.MIN)
+        host_ok = bool(flag.item())
+    seed = SEED + 1000 * rank
+    if host_ok:
+        h_in = torch.empty(shape, dtype=torch.complex128).pin_memory()
+        inputs.uniform_pm1(shape, seed, out=h_in.numpy())
+        h_out = torch.empty(shape, dtype=torch.complex128).pin_memory()
+        d_in = h_in.cuda()
+    else:
+        h_in = h_out = None
+        d_in = torch.empty(shape, dtype=torch.complex128, device="cuda")
+        flat = d_in.view(torch.float64).view(-1)
+        step = 1 << 26
+        for s0 in range(0, 2 * n_tot, step):
+            c = min(step, 2 * n_tot - s0)
+            flat[s0:s0 + c].copy_(torch.from_numpy(2.0 * inputs.uniform01(seed, s0, c) - 1.0))
     d_out = torch.empty_like(d_in)
     plan = ozfft.Plan(size, size, size, sign=-1)
     launches = plan.num_launches
@@ -195,16 +216,20 @@ def run_ours(args):
 
     # end to end through the public API with HOST buffers
     e2e_steps = max(1, min(args.steps, 3))
-    plan.exec_host(h_in, h_out)  # warm-up (allocates the staging buffers)
-    barrier()
-    t0 = time.perf_counter()
-    for _ in range(e2e_steps):
-        plan.exec_host(h_in, h_out)
-    barrier()
-    e2e_ms = (time.perf_counter() - t0) * 1e3 / e2e_steps
+    e2e_ms, same = float("nan"), None
+    if host_ok:
+        plan.exec_host(h_in, h_out)  # warm-up (allocates the staging buffers)
+        barrier()
+        t0 = time.perf_counter()
+        for _ in range(e2e_steps):
+            plan.exec_host(h_in, h_out)
+        barrier()
+        e2e_ms = (time.perf_counter() - t0) * 1e3 / e2e_steps
+        # sanity inside the bench: device-resident and host paths agree bit for bit
+        same = bool(torch.equal(d_out.cpu().view(torch.float64), h_out.view(torch.float64)))
 
-    # sanity inside the bench: device-resident and host paths agree bit for bit; round trip
-    same = bool(torch.equal(d_out.cpu().view(torch.float64), h_out.view(torch.float64)))
+    # round trip (BASELINE.json configs[4]: forward then inverse)
+    x_keep = d_in.view(-1)[: min(n_tot, 1 << 27)].clone()
     inv = ozfft.Plan(size, size, size, sign=+1)
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     e0.record(stream)
@@ -213,20 +238,20 @@ def run_ours(args):
     torch.cuda.synchronize()
     inv_ms = e0.elapsed_time(e1)
     chunk = 1 << 24
-    flat_rt, flat_x = d_in.view(-1), h_in.view(-1)
+    flat_rt = d_in.view(-1)
     num = den = 0.0
-    for s in range(0, min(n_tot, 1 << 27), chunk):
+    for s in range(0, x_keep.numel(), chunk):
         a = flat_rt[s:s + chunk] / n_tot
-        b = flat_x[s:s + chunk].cuda()
+        b = x_keep[s:s + chunk]
         num += float(((a - b).abs() ** 2).sum())
         den += float((b.abs() ** 2).sum())
     roundtrip = math.sqrt(num / den)
     inv.destroy()
+    del x_keep
 
     # cuFFT Z2Z context number (not part of the path)
     cufft_ms = None
     try:
-        d_in.copy_(h_in, non_blocking=False)
         for _ in range(2):
             y = torch.fft.fftn(d_in)
             del y
@@ -240,7 +265,7 @@ def run_ours(args):
     except Exception as ex:  # out of memory at the largest size is not fatal for the bench line
         cufft_ms = None
 
-    ms_step_max, e2e_ms_max = max_over_ranks([ms_step, e2e_ms], device="cuda")
+    ms_step_max, e2e_ms_max = max_over_ranks([ms_step, e2e_ms if host_ok else 0.0], device="cuda")
 
     if rank == 0:
         peak, peak_src = peaks()
@@ -262,8 +287,10 @@ def run_ours(args):
                          "traffic": NCU_TRAFFIC_PER_LAUNCH.get(size), "kernel": "stage kernel (all launches of a transform are this kernel)",
                          "peak_source": peak_src, "alg_bytes_per_launch": alg_bytes_launch, "launch_ms": launch_ms},
             "clocks": clocks,
-            "e2e": {"value": world * flops(n_tot) / (e2e_ms_max * 1e-3) / 1e9, "unit": "GFLOP/s", "ms": e2e_ms_max,
-                    "h2d_bytes_per_step": nbytes, "d2h_bytes_per_step": nbytes, "steps": e2e_steps},
+            "e2e": ({"value": world * flops(n_tot) / (e2e_ms_max * 1e-3) / 1e9, "unit": "GFLOP/s", "ms": e2e_ms_max,
+                     "h2d_bytes_per_step": nbytes, "d2h_bytes_per_step": nbytes, "steps": e2e_steps} if host_ok else
+                    {"value": None, "unit": "GFLOP/s", "h2d_bytes_per_step": nbytes, "d2h_bytes_per_step": nbytes,
+                     "skipped": "not enough host memory on this node for N x 2 x 16 GiB of pinned buffers"}),
             "gpu_launches": launches * args.steps,
             # what actually binds: SIMT integer issue.  achieved = n_out x the ncu-measured thread
             # instructions per output-equivalent (profiles/r1_final.md) / step time; peak = 148 SM x 128 lanes x 1.965 GHz
