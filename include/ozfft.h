@@ -56,6 +56,18 @@ int ozfft_exec_axis(ozfft_plan plan, int axis, const void *in, void *out, void *
  * M=128 tcgen05.mma of K = 32 bytes each.  kind 0: f8f6f4 E4M3 -> f32; 1: f16 -> f32; 2: i8 (s8) -> s32;
  * 3: f16 with A fed from TMEM; 4: i8 (u8 x u8) -> s32.  All pointers device.  n multiple of 16 in [16,256], kbytes multiple of 32. */
 int ozfft_probe_mma(int kind, int n, int kbytes, const void *dA, const void *dB, void *dD, void *stream);
+/* Chained probe: D1[128][n1] = A[128][kbytes] * B1[n1][kbytes]^T (u8 x u8 -> s32, kept in TMEM), then
+ * D2[128][n2] = bytes(D1)[128][4 n1] * B2[n2][4 n1]^T with the second MMA reading its A operand straight from the
+ * TMEM accumulator of the first (K byte 4c+b = little-endian byte b of D1[.][c]).  The byte-fed stage kernel uses
+ * exactly this to run Phase A on the stage accumulators without a SIMT pass.  Device pointers. */
+int ozfft_probe_chain(int n1, int kbytes, int n2, const void *dA, const void *dB1, const void *dB2, void *dD1, void *dD2,
+                      void *stream);
+/* Device CRT probe (PAPER.md:316-329 direct CRT, 370-373 two-sided lift, Alg. 2 lines 9-13 at 408-413):
+ * d_residues = n x 12 uint16 (any representative of each residue below 2^13), d_out = n x 4 uint32 = two's-complement
+ * limbs of the centred result in [-M/2, M/2).  variant 1: the tensor-core form the stage kernels use (Phase-A MMA,
+ * deposits, quotient from the top of E, two-sided centring); variant 0: the SIMT kernel's 128-bit form.
+ * Synchronises `stream`.  Device pointers. */
+int ozfft_probe_crt(int n, const void *d_residues, void *d_out, int variant, void *stream);
 
 #ifdef __cplusplus
 }

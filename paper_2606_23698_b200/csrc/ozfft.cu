@@ -14,6 +14,7 @@
 #include "stage_simt.cuh"
 #include "stage_tc.cuh"
 #include "tables.cuh"
+#include "probe.cuh"
 
 using namespace oz;
 
@@ -444,6 +445,21 @@ void ozfft_plan_destroy(ozfft_plan p) {
 }
 
 const char *ozfft_last_error(void) { return g_err.c_str(); }
+
+int ozfft_probe_crt(int n, const void *d_residues, void *d_out, int variant, void *stream) {
+    if (n <= 0 || !d_residues || !d_out || (variant != 0 && variant != 1)) { set_err("ozfft_probe_crt: bad argument"); return OZFFT_EINVAL; }
+    DevConsts hc;
+    fill_consts(hc);
+    DevConsts *dc = nullptr;
+    if (!cuda_ok(cudaMalloc(&dc, sizeof(hc)), "cudaMalloc(consts)")) return OZFFT_ECUDA;
+    bool ok = cuda_ok(cudaMemcpy(dc, &hc, sizeof(hc), cudaMemcpyHostToDevice), "cudaMemcpy(consts)") && stage_tc_prepare(hc);
+    if (ok) {
+        probe_crt_kernel<<<(unsigned)((n + 127) / 128), 128, 0, (cudaStream_t)stream>>>(variant, n, (const uint16_t *)d_residues, (uint32_t *)d_out, dc);
+        ok = cuda_ok(cudaGetLastError(), "probe_crt_kernel launch") && cuda_ok(cudaStreamSynchronize((cudaStream_t)stream), "probe_crt_kernel");
+    }
+    cudaFree(dc);
+    return ok ? OZFFT_OK : OZFFT_ECUDA;
+}
 
 uint64_t ozfft_twiddle_checksum(void) { return twiddle_fnv(twiddles()); }
 

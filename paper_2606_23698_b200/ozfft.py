@@ -12,7 +12,7 @@ _lib = None
 
 SYMBOLS = ["ozfft_plan_create", "ozfft_plan_create_1d", "ozfft_exec", "ozfft_exec_host", "ozfft_plan_destroy",
            "ozfft_last_error", "ozfft_twiddle_checksum", "ozfft_plan_num_launches", "ozfft_plan_device_bytes",
-           "ozfft_exec_axis", "ozfft_probe_mma"]
+           "ozfft_exec_axis", "ozfft_probe_mma", "ozfft_probe_chain", "ozfft_probe_crt"]
 
 
 def lib():
@@ -37,6 +37,8 @@ def lib():
         L.ozfft_plan_device_bytes.argtypes = [vp]
         L.ozfft_plan_device_bytes.restype = C.c_size_t
         L.ozfft_probe_mma.argtypes = [C.c_int, C.c_int, C.c_int, vp, vp, vp, vp]
+        L.ozfft_probe_chain.argtypes = [C.c_int, C.c_int, C.c_int, vp, vp, vp, vp, vp, vp]
+        L.ozfft_probe_crt.argtypes = [C.c_int, vp, vp, C.c_int, vp]
         _lib = L
     return _lib
 
@@ -129,3 +131,28 @@ def probe_mma(kind, A, B):
     _check(lib().ozfft_probe_mma(kind, n, kb, A.data_ptr(), B.data_ptr(), D.data_ptr(), _stream(None)), "ozfft_probe_mma")
     torch.cuda.synchronize()
     return D
+
+
+def probe_chain(A, B1, B2):
+    """A: uint8 CUDA [128, kb]; B1: uint8 [n1, kb]; B2: uint8 [n2, 4*n1] -> (D1 int32 [128, n1], D2 int32 [128, n2]):
+    D2 = bytes(D1) @ B2^T with the second MMA's A operand read from the TMEM accumulator of the first."""
+    import torch
+    n1, kb = B1.shape
+    n2 = B2.shape[0]
+    assert B2.shape[1] == 4 * n1
+    D1 = torch.zeros((128, n1), dtype=torch.int32, device=A.device)
+    D2 = torch.zeros((128, n2), dtype=torch.int32, device=A.device)
+    _check(lib().ozfft_probe_chain(n1, kb, n2, A.data_ptr(), B1.data_ptr(), B2.data_ptr(), D1.data_ptr(), D2.data_ptr(),
+                                   _stream(None)), "ozfft_probe_chain")
+    torch.cuda.synchronize()
+    return D1, D2
+
+
+def probe_crt(residues, variant):
+    """residues: uint16 CUDA tensor [n, 12] -> int32 CUDA [n, 4]: two's-complement limbs of the centred CRT result."""
+    import torch
+    n = residues.shape[0]
+    assert residues.dtype == torch.uint16 and residues.shape[1] == 12 and residues.is_contiguous()
+    out = torch.zeros((n, 4), dtype=torch.int32, device=residues.device)
+    _check(lib().ozfft_probe_crt(n, residues.data_ptr(), out.data_ptr(), variant, _stream(None)), "ozfft_probe_crt")
+    return out

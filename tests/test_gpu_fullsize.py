@@ -13,16 +13,17 @@ def _bits(a):
     return np.ascontiguousarray(a).view(np.uint64)
 
 
-def test_config3_batched_1d_full(O):
+@pytest.mark.parametrize("sign", [-1, +1])
+def test_config3_batched_1d_full(O, sign):
     import torch
     from paper_2606_23698_b200 import inputs, ozfft
     x = inputs.normal((65536, 1024), 2)
-    plan = ozfft.Plan.batched_1d(1024, 65536)
+    plan = ozfft.Plan.batched_1d(1024, 65536, sign=sign)
     got = plan.exec(torch.from_numpy(x).cuda()).cpu().numpy()
     plan.destroy()
-    want, bad = O.fft1d(x, -1, route=0)
+    want, bad = O.fft1d(x, sign, route=0)
     assert np.array_equal(_bits(got), _bits(want))
-    assert O.relerr_1d_f128(x[:16], got[:16]) <= 5e-15
+    assert O.relerr_1d_f128(x[:16], got[:16], sign) <= 5e-15
 
 
 def test_config4_512cubed_full(O):
@@ -71,10 +72,24 @@ def test_config5_1024cubed_sampled_passes_and_roundtrip(O):
     idx = np.sort(rng.choice(n ** 3, 3, replace=False)).astype(np.int64)
     ys = full.view(-1)[torch.from_numpy(idx).cuda()].cpu().numpy()
     assert O.relerr_3d_f128(h.numpy(), idx, ys) <= 5e-15
-    # forward then inverse (configs[4]): round-trip error
+    # forward then inverse (configs[4]): the inverse passes are bit-checked the same way (sampled pencils of each
+    # pass against the oracle's sign=+1 transform), then the round-trip error
     inv = ozfft.Plan(n, n, n, sign=+1)
+    cur = full
+    for axis in range(3):
+        nxt = inv.exec_axis(axis, cur)
+        torch.cuda.synchronize()
+        for _ in range(32):
+            a, b = (int(v) for v in rng.integers(0, n, 2))
+            sl = (a, b, slice(None)) if axis == 0 else ((a, slice(None), b) if axis == 1 else (slice(None), a, b))
+            assert np.array_equal(_bits(nxt[sl].cpu().numpy()), _bits(O.fft1d_pencil(cur[sl].cpu().numpy(), +1))), (axis, a, b)
+        if axis:
+            del cur
+        cur = nxt
     back = inv.exec(full)
     torch.cuda.synchronize()
+    assert torch.equal(back.view(torch.float64), cur.view(torch.float64))
+    del cur
     num = den = 0.0
     for i in range(0, n, 64):
         d = back[i:i + 64] / float(n ** 3) - x[i:i + 64]

@@ -95,13 +95,15 @@ def test_inverse_and_roundtrip(O):
     assert np.linalg.norm(z / x.size - x) / np.linalg.norm(x) < 5e-15
 
 
+@pytest.mark.parametrize("sign", [-1, +1])
 @pytest.mark.parametrize("n", [1024, 512, 64, 32, 8])
-def test_batched_1d_bit_exact(O, n):
+def test_batched_1d_bit_exact(O, n, sign):
+    """both directions at every fused-stage width (second-stage K = 32, 16, 2, -, -)"""
     from paper_2606_23698_b200 import inputs
     x = inputs.normal((96, n), 2)
-    got = _run1d(x)
-    _assert_bit_exact(got, O.fft1d(x, -1, route=0)[0])
-    assert O.relerr_1d_f128(x[:8], got[:8]) <= TOL_F128
+    got = _run1d(x, sign)
+    _assert_bit_exact(got, O.fft1d(x, sign, route=0)[0])
+    assert O.relerr_1d_f128(x[:8], got[:8], sign) <= TOL_F128
 
 
 def test_edge_columns_zero_subnormal_huge(O):

@@ -70,3 +70,23 @@ def test_u8_phase_a_two_limb_contract():
     B[0] = 255
     D = _probe(4, A, B)
     assert np.array_equal(D, A.astype(np.int64) @ B.astype(np.int64).T) and D.max() == 32 * 255 * 255
+
+
+@pytest.mark.parametrize("n1,kb,n2", [(16, 32, 16), (48, 224, 32), (96, 448, 32)])
+def test_i8_mma_reads_s32_accumulators_from_tmem_as_bytes(n1, kb, n2):
+    """The byte-fed stage kernel runs Phase A with its A operand read straight from the stage
+    accumulators in TMEM: a 32-bit cell must act as four unsigned K bytes, little endian, K byte = 4*column + b."""
+    import torch
+    from paper_2606_23698_b200 import ozfft
+    rng = np.random.default_rng(n1 + kb + n2)
+    A = rng.integers(0, 256, (128, kb), dtype=np.uint8)
+    B1 = rng.integers(0, 256, (n1, kb), dtype=np.uint8)
+    A[0] = 255
+    B1[0] = 255
+    B2 = rng.integers(0, 256, (n2, 4 * n1), dtype=np.uint8)
+    D1, D2 = ozfft.probe_chain(torch.from_numpy(A).cuda(), torch.from_numpy(B1).cuda(), torch.from_numpy(B2).cuda())
+    D1, D2 = D1.cpu().numpy(), D2.cpu().numpy()
+    want1 = A.astype(np.int64) @ B1.astype(np.int64).T
+    assert np.array_equal(D1, want1)
+    by = np.ascontiguousarray(want1.astype(np.uint32)).view(np.uint8).reshape(128, 4 * n1)  # little-endian bytes
+    assert np.array_equal(D2, by.astype(np.int64) @ B2.astype(np.int64).T)

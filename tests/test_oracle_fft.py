@@ -175,6 +175,39 @@ def test_fft3d_small_full_checks(O):
     assert np.linalg.norm(back / x1.size - x1) / np.linalg.norm(x1) < 5e-15
 
 
+def test_fft3d_two_stage_axes_pinned(O):
+    """3-D with two-stage axes (n > 32: q = 32 first stage, p = n/32 twiddle-fused second stage, PAPER.md:115-124,
+    210-214) on 64 x 32 x 64, residue route (route 2): (i) bit-identical to composing the 1-D transform (itself pinned
+    to the __float128 DFT above) along z, y, x with the array rounded to fp64 between passes (reading
+    S6) -- a wrong stride, axis order or stage index in the 3-D driver fails here; (ii) <= 5e-15 against the
+    __float128 3-D DFT on 512 sampled outputs; (iii) closed forms: off-origin impulse, DC."""
+    shape = (64, 32, 64)
+    x = inputs.uniform_pm1(shape, seed=5)
+    O.reset_capacity_violations()
+    y, bad = O.fft3d(x, -1, route=2)
+    assert bad == 0 and O.capacity_violations() == 0
+    comp = x
+    for axis in (2, 1, 0):
+        moved = np.ascontiguousarray(np.moveaxis(comp, axis, -1))
+        t, bad1 = O.fft1d(moved.reshape(-1, shape[axis]), -1, route=0)
+        assert bad1 == 0
+        comp = np.ascontiguousarray(np.moveaxis(t.reshape(moved.shape), -1, axis))
+    assert np.array_equal(bits(y), bits(comp))
+    rng = np.random.default_rng(1)
+    idx = np.sort(rng.choice(x.size, 512, replace=False)).astype(np.int64)
+    assert O.relerr_3d_f128(x, idx, y.reshape(-1)[idx], -1) <= 5e-15
+    yi, _ = O.fft3d(y, +1, route=0)
+    assert np.linalg.norm(yi / x.size - x) / np.linalg.norm(x) < 5e-15
+    imp = np.zeros(shape, dtype=np.complex128); imp[5, 3, 41] = 1.0
+    yimp, _ = O.fft3d(imp, -1)
+    kx, ky, kz = np.meshgrid(np.arange(64), np.arange(32), np.arange(64), indexing="ij")
+    want = np.exp(-2j * np.pi * (((5 * kx + 6 * ky + 41 * kz) % 64) / 64))
+    assert np.abs(yimp - want).max() < 1e-15
+    yd, _ = O.fft3d(np.ones(shape, dtype=np.complex128), -1)
+    want = np.zeros(shape, dtype=np.complex128); want[0, 0, 0] = x.size
+    assert np.array_equal(bits(yd), bits(want))
+
+
 def test_lograng_dynamic_range_config2_slice(O):
     """Config 2's distribution (|x| log-uniform in 2^+-30) on a 1-D batch: capacity never trips,
     residue route == direct, accuracy bound holds."""
