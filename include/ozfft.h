@@ -56,6 +56,12 @@ int ozfft_exec_axis(ozfft_plan plan, int axis, const void *in, void *out, void *
  * M=128 tcgen05.mma of K = 32 bytes each.  kind 0: f8f6f4 E4M3 -> f32; 1: f16 -> f32; 2: i8 (s8) -> s32;
  * 3: f16 with A fed from TMEM; 4: i8 (u8 x u8) -> s32.  All pointers device.  n multiple of 16 in [16,256], kbytes multiple of 32. */
 int ozfft_probe_mma(int kind, int n, int kbytes, const void *dA, const void *dB, void *dD, void *stream);
+/* Host-only table export of the byte-fed stage kernel (no GPU needed; tests/test_bf_tables_cpu.py emulates the
+ * kernel's integer dataflow on these tables and compares with the oracle's stage).  K = contraction length,
+ * fusedN = 0 (plain DFT_K) or 32*K (twiddle-fused second stage, Eq. 6).  HOST pointers, any may be
+ * NULL: h_B receives the matrix byte planes (return value = their size in bytes, 0 on a bad argument), h_C the
+ * offset constants (nmat*K*16 bytes), h_PA the Phase-A constant matrix (6144 bytes).  Layouts: csrc/stage_bf.cuh. */
+size_t ozfft_debug_bf_tables(int K, int fusedN, int sign, void *h_B, void *h_C, void *h_PA);
 /* Chained probe: D1[128][n1] = A[128][kbytes] * B1[n1][kbytes]^T (u8 x u8 -> s32, kept in TMEM), then
  * D2[128][n2] = bytes(D1)[128][4 n1] * B2[n2][4 n1]^T with the second MMA reading its A operand straight from the
  * TMEM accumulator of the first (K byte 4c+b = little-endian byte b of D1[.][c]).  The byte-fed stage kernel uses

@@ -225,6 +225,18 @@ __device__ __forceinline__ void deposit_slices(const uint32_t *P, uint32_t *r) {
     crt_from_E((uint32_t)w[0], (uint32_t)t1, (uint32_t)t2, (uint32_t)t3, (uint32_t)(t3 >> 32), r);
 }
 
+// the same deposits, returning the five limbs of E (the byte-fed kernel lifts later, after freeing its TMEM slot)
+__device__ __forceinline__ void slices_to_E(const uint32_t *P, uint32_t *e) {
+    uint64_t w[4];
+#pragma unroll
+    for (int j = 0; j < 4; j++) {
+        w[j] = (uint64_t)P[4 * j + 2] * 65536u + (P[4 * j] + P[4 * j + 1] * 256u);
+        w[j] = (uint64_t)P[4 * j + 3] * 16777216u + w[j];
+    }
+    const uint64_t t1 = (w[0] >> 32) + w[1], t2 = (t1 >> 32) + w[2], t3 = (t2 >> 32) + w[3];
+    e[0] = (uint32_t)w[0]; e[1] = (uint32_t)t1; e[2] = (uint32_t)t2; e[3] = (uint32_t)t3; e[4] = (uint32_t)(t3 >> 32);
+}
+
 // lift and centring from the limbs of E (< 2^134): see crt_limbs
 __device__ __forceinline__ void crt_from_E(uint32_t e0, uint32_t e1, uint32_t e2, uint32_t e3, uint32_t e4, uint32_t *r) {
     const uint32_t T = __funnelshift_r(e3, e4, 8);  // E >> 104

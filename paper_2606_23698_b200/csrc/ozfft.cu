@@ -13,6 +13,7 @@
 #include "stage.cuh"
 #include "stage_simt.cuh"
 #include "stage_tc.cuh"
+#include "stage_bf.cuh"
 #include "tables.cuh"
 #include "probe.cuh"
 
@@ -39,6 +40,8 @@ struct StageLaunch {
     StageGeom g;
     const ushort2 *mat_simt;  // [nmat][12][K][K] (a_R, a_I) canonical residues
     const uint8_t *mat_tc;    // digit planes for the tensor-core kernel (stage_tc.cuh)
+    const uint8_t *mat_bf;    // matrix byte planes of the byte-fed kernel (stage_bf.cuh)
+    const void *ctab_bf;      // its offset constants [nmat][K] x 16 B
     int axis;
 };
 
@@ -48,7 +51,9 @@ struct ozfft_plan_s {
     uint32_t magic;
     int nx, ny, nz, sign;
     long long count;
-    int variant;  // 0 simt, 1 tensor-core
+    int variant;  // 0 simt, 1 tensor-core (residue digits), 2 byte-fed tensor-core (default)
+    int sms;      // SM count of the plan's device
+    const void *pa_bf;  // Phase-A constant matrix of the byte-fed kernel
     std::vector<StageLaunch> stages;
     std::vector<void *> dev_allocs;
     size_t dev_bytes;
@@ -132,6 +137,12 @@ struct MatKey {
     int K, fusedN;
     bool operator<(const MatKey &o) const { return K != o.K ? K < o.K : fusedN < o.fusedN; }
 };
+struct MatSet {
+    const ushort2 *simt;
+    const uint8_t *tc, *bf;
+    const void *ctab;
+};
+typedef std::map<MatKey, MatSet> MatMap;
 
 void *dev_upload(ozfft_plan_s *p, const void *src, size_t bytes) {
     void *d = nullptr;
@@ -164,8 +175,7 @@ struct AxisDesc {
     long long outer, N, inner;  // strided: element (o, i, z) at (o*N + i)*inner + z; contiguous: pencil P at P*N
 };
 
-bool add_axis(ozfft_plan_s *p, const AxisDesc &a, int axis, std::map<MatKey, std::pair<const ushort2 *, const uint8_t *>> &mats,
-              std::vector<StageLaunch> &dst) {
+bool add_axis(ozfft_plan_s *p, const AxisDesc &a, int axis, MatMap &mats, std::vector<StageLaunch> &dst) {
     const int N = (int)a.N;
     const bool two = N > 32;
     const int q = two ? 32 : N, pp = two ? N / 32 : 1;
@@ -173,19 +183,29 @@ bool add_axis(ozfft_plan_s *p, const AxisDesc &a, int axis, std::map<MatKey, std
         MatKey key{K, fusedN};
         auto it = mats.find(key);
         if (it == mats.end()) {
-            const ushort2 *ms = build_mat_simt(p, K, fusedN);
-            if (!ms) return false;
-            const uint8_t *mt = nullptr;
-            if (p->variant == 1) {
+            MatSet ms{};
+            if (p->variant == 0) {
+                ms.simt = build_mat_simt(p, K, fusedN);
+                if (!ms.simt) return false;
+            } else if (p->variant == 1) {
                 std::vector<uint8_t> h;
                 build_mat_tc(h, K, fusedN, p->sign, twiddles());
-                mt = (const uint8_t *)dev_upload(p, h.data(), h.size());
-                if (!mt) return false;
+                ms.tc = (const uint8_t *)dev_upload(p, h.data(), h.size());
+                if (!ms.tc) return false;
+            } else {
+                std::vector<uint8_t> h;
+                std::vector<uint32_t> c;
+                build_mat_bf(h, c, K, fusedN, p->sign, twiddles());
+                ms.bf = (const uint8_t *)dev_upload(p, h.data(), h.size());
+                ms.ctab = dev_upload(p, c.data(), c.size() * 4);
+                if (!ms.bf || !ms.ctab) return false;
             }
-            it = mats.insert({key, {ms, mt}}).first;
+            it = mats.insert({key, ms}).first;
         }
-        s.mat_simt = it->second.first;
-        s.mat_tc = it->second.second;
+        s.mat_simt = it->second.simt;
+        s.mat_tc = it->second.tc;
+        s.mat_bf = it->second.bf;
+        s.ctab_bf = it->second.ctab;
         return true;
     };
     StageLaunch s1{}, s2{};
@@ -227,7 +247,8 @@ bool add_axis(ozfft_plan_s *p, const AxisDesc &a, int axis, std::map<MatKey, std
 int pick_variant() {
     const char *v = getenv("OZFFT_VARIANT");
     if (v && !strcmp(v, "simt")) return 0;
-    return 1;
+    if (v && !strcmp(v, "tc")) return 1;
+    return 2;
 }
 
 ozfft_plan_s *make_plan(int nx, int ny, int nz, int sign, bool batched1d) {
@@ -249,8 +270,18 @@ ozfft_plan_s *make_plan(int nx, int ny, int nz, int sign, bool batched1d) {
     DevConsts hc;
     fill_consts(hc);
     p->d_consts = (DevConsts *)dev_upload(p, &hc, sizeof(hc));
-    std::map<MatKey, std::pair<const ushort2 *, const uint8_t *>> mats;
+    MatMap mats;
     bool ok = p->d_consts != nullptr;
+    p->sms = prop.multiProcessorCount;
+    p->pa_bf = nullptr;
+    if (ok && p->variant == 2) {
+        CrtConsts C;
+        build_crt(C);
+        std::vector<uint8_t> pa(BF_PA_BYTES);
+        build_pa_bf(pa.data(), C);
+        p->pa_bf = dev_upload(p, pa.data(), pa.size());
+        ok = p->pa_bf != nullptr;
+    }
     if (batched1d) {  // nx = batch, nz = n
         ok = ok && add_axis(p, AxisDesc{true, nx, nz, 1}, 0, mats, p->stages);
     } else {
@@ -270,7 +301,9 @@ ozfft_plan_s *make_plan(int nx, int ny, int nz, int sign, bool batched1d) {
         ok = cuda_ok(cudaMalloc(&p->work, (size_t)p->count * 16), "cudaMalloc(workspace)");
         if (ok) p->dev_bytes += (size_t)p->count * 16;
     }
-    if (ok && p->variant == 1) ok = stage_tc_prepare(hc);
+    if (ok && p->variant >= 1) ok = stage_tc_prepare(hc);  // uploads the constant bank both tensor-core kernels read
+    if (ok && p->variant == 2) ok = stage_bf_prepare();
+    if (!ok && g_err.empty()) set_err("kernel attribute setup failed");
     if (!ok) {
         std::string keep = g_err;
         ozfft_plan_destroy(p);
@@ -284,7 +317,16 @@ bool valid(ozfft_plan p) { return p && p->magic == PLAN_MAGIC; }
 
 int launch_stage(ozfft_plan p, const StageLaunch &s, const void *src, void *dst, cudaStream_t st) {
     const long long nt = (long long)s.g.nb * s.g.ns * s.g.no;
-    if (p->variant == 1) return stage_tc_launch(s.g, src, dst, s.mat_tc, p->d_consts, st) ? OZFFT_OK : OZFFT_ECUDA;
+    if (p->variant == 2) {
+        if (stage_bf_launch(s.g, src, dst, s.mat_bf, s.ctab_bf, p->pa_bf, p->sms, st)) return OZFFT_OK;
+        set_err(std::string("stage_bf_kernel launch: ") + cudaGetErrorString(cudaGetLastError()));
+        return OZFFT_ECUDA;
+    }
+    if (p->variant == 1) {
+        if (stage_tc_launch(s.g, src, dst, s.mat_tc, p->d_consts, st)) return OZFFT_OK;
+        set_err(std::string("stage_tc_kernel launch: ") + cudaGetErrorString(cudaGetLastError()));
+        return OZFFT_ECUDA;
+    }
     const size_t sm = (size_t)s.g.K * 32 * 16 + (size_t)12 * s.g.K * 32 * 4;
     static bool attr = false;
     if (!attr) {
@@ -459,6 +501,21 @@ int ozfft_probe_crt(int n, const void *d_residues, void *d_out, int variant, voi
     }
     cudaFree(dc);
     return ok ? OZFFT_OK : OZFFT_ECUDA;
+}
+
+size_t ozfft_debug_bf_tables(int K, int fusedN, int sign, void *h_B, void *h_C, void *h_PA) {
+    if (K < 2 || K > 32 || (K & (K - 1)) || (sign != 1 && sign != -1) || (fusedN && fusedN != 32 * K)) return 0;
+    std::vector<uint8_t> B;
+    std::vector<uint32_t> Cc;
+    build_mat_bf(B, Cc, K, fusedN, sign, twiddles());
+    if (h_B) memcpy(h_B, B.data(), B.size());
+    if (h_C) memcpy(h_C, Cc.data(), Cc.size() * 4);
+    if (h_PA) {
+        CrtConsts C;
+        build_crt(C);
+        build_pa_bf((uint8_t *)h_PA, C);
+    }
+    return B.size();
 }
 
 uint64_t ozfft_twiddle_checksum(void) { return twiddle_fnv(twiddles()); }

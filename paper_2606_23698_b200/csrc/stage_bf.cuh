@@ -1,0 +1,443 @@
+// stage_bf.cuh -- "byte-fed" stage kernel: one Bailey stage whose per-modulus work runs entirely on tcgen05.
+//
+// Idea (what differs from the paper's sketch, and from stage_tc.cuh): the DATA operand of the
+// stage GEMM is not a residue plane but the raw bytes of the quantised 54-bit integers, w = x~ + 2^53 =
+// sum_b w_b 256^b (7 unsigned bytes), so it is the SAME for all twelve moduli and is written once per tile.
+// The modulus-dependent part moves into the MATRIX operand: for modulus m_i, entry (k, j, h, b) is the
+// two-byte split (digit d = 0, 1) of  c_{kjh} 256^b mod m_i,  c = a_R (h = 0) or a_I (h = 1)
+// ("sum_k b_k (2^{8k} mod m_i)" folded into the DFT matrix, Eq. 6 for the fused one).
+// One u8 x u8 -> s32 MMA therefore yields, per (column, output, modulus), two accumulators lo, hi with
+// lo + 256 hi == sum_j c_kj w_j (mod m_i): deconstruction (a3), the residue GEMM (a4) and the recombination (a5)
+// are one tensor-core operation, and no per-modulus SIMT instruction exists.
+//
+// Rows: MMA row r = data column r.  The re part contracts [x_R ; -x_I] and the im part [x_I ; x_R] against the one
+// matrix [a_R ; a_I] (direct 4-product complex form): three byte planes XI, XR, NXI (-x_I) per tile serve both.
+// Radix-2 in the output index: with H = K/2, a~_{k+H,j} = (-1)^j a~_{k,j} holds EXACTLY in the quantised table
+// (T[t+512] = -T[t], reading S5), so the even-j and odd-j partial sums S^E_k, S^O_k (k < H) are accumulated
+// separately (half the matrix, half the MMA work) and out_k = S^E + S^O, out_{k+H} = S^E - S^O are formed inside
+// Phase A, which is linear: its constant matrix carries u_i for the sum and M - u_i for the difference.
+//
+// Phase A (tc-CRT, two-limb form 759-764, here a byte-limb form): the s32 stage accumulators
+// stay in TMEM and ARE the A operand of a second kind::i8 MMA (a 32-bit TMEM cell = four unsigned K bytes; contract
+// measured by tests/test_gpu_silicon.py): P_s = sum_{i,d,b} byte_b(acc_{i,d}) * byte_s(256^{d+b} u_i mod M).
+// Phase B (Alg. 2): deposits E = sum_s P_s 256^s, lift, two-sided centring (arith.cuh), minus the
+// offset constant C_k = 2^53 sum_j (a_R + a_I)_kj, one RNE pack to fp64.
+//
+// Capacity: |R + C| <= 2^111.5 + 2^111.5 < M/2 = 2^116.9.  E < 30768 M < 2^134.
+#pragma once
+#include <vector>
+
+#include "arith.cuh"
+#include "stage.cuh"
+#include "tables.cuh"
+#include "tc.cuh"
+
+namespace oz {
+
+// ---- geometry of the operands for contraction length K (2..32, power of two)
+__host__ __device__ constexpr int bf_H(int K) { return K / 2; }                                 // output pairs (k, k + H)
+__host__ __device__ constexpr int bf_PB(int K) { return ((7 * (K / 2) + 15) / 16) * 16; }       // bytes of one (plane, parity) block
+__host__ __device__ constexpr int bf_NCK(int K) { return bf_PB(K) / 16; }                       // its 16-byte chunks = K steps of a chain
+__host__ __device__ constexpr int bf_NCH(int K) { return (K / 2 + 1) / 2; }                     // matrix chunks (2 pairs each) per tile
+constexpr int BF_N = 48;            // stage MMA N: 2 pairs x 12 moduli x 2 digits
+constexpr int BF_COLS = 128;        // data columns per tile = MMA M
+constexpr int BF_PA_BYTES = 32 * 192;  // Phase-A constant matrix: N = 2 outputs x 16 slices, K = (E|O) x 12 x 2 x 4 bytes
+__host__ __device__ constexpr int bf_slot_bytes(int K) { return BF_N * 2 * bf_PB(K); }          // one parity of one chunk
+__host__ __device__ constexpr int bf_plane_bytes(int K) { return 2 * bf_NCK(K) * BF_COLS * 16; }  // both parities
+__host__ __device__ constexpr int bf_aset_bytes(int K) { return 3 * bf_plane_bytes(K); }        // XI, XR, NXI
+__host__ __device__ constexpr size_t bf_mat_bytes(int K) { return (size_t)bf_NCH(K) * 2 * bf_slot_bytes(K); }  // per matrix id
+
+inline int bf_tw_index(int K, int fusedN, int mid, int k, int j) {
+    if (!fusedN) return (int)(((long)(TABLE_N / K) * j * k) % TABLE_N);
+    return (int)(((long)(TABLE_N / fusedN) * j * (mid + 32L * k)) % TABLE_N);
+}
+
+// host: matrix byte planes for all matrix ids: [mid][chunk][parity][kappa/16][n = g*24 + i*2 + d][16 B], kappa =
+// h*PB + jj*7 + b for element j = 2 jj + parity, half h, byte b; and the offset constants C[mid][k] (two's complement,
+// four 32-bit limbs) = 2^53 * sum_j (a_R + a_I)_{kj}.
+inline void build_mat_bf(std::vector<uint8_t> &B, std::vector<uint32_t> &Cc, int K, int fusedN, int sign, const Twiddles &T) {
+    const int H = bf_H(K), PB = bf_PB(K), NCH = bf_NCH(K), nmat = fusedN ? 32 : 1, SB = bf_slot_bytes(K);
+    B.assign((size_t)nmat * bf_mat_bytes(K), 0);
+    Cc.assign((size_t)nmat * K * 4, 0);
+    int p256[R_MOD][7];
+    for (int i = 0; i < R_MOD; i++) {
+        p256[i][0] = 1 % kModuli[i];
+        for (int b = 1; b < 7; b++) p256[i][b] = (p256[i][b - 1] * 256) % kModuli[i];
+    }
+    for (int mid = 0; mid < nmat; mid++) {
+        for (int k = 0; k < K; k++) {
+            __int128 s = 0;
+            for (int j = 0; j < K; j++) {
+                const int t = bf_tw_index(K, fusedN, mid, k, j);
+                s += (__int128)T.c[t] + (__int128)sign * T.s[t];
+            }
+            const unsigned __int128 c = (unsigned __int128)(s * ((__int128)1 << 53));
+            for (int l = 0; l < 4; l++) Cc[((size_t)mid * K + k) * 4 + l] = (uint32_t)(c >> (32 * l));
+        }
+        for (int ch = 0; ch < NCH; ch++)
+            for (int par = 0; par < 2; par++) {
+                uint8_t *dst = B.data() + (size_t)mid * bf_mat_bytes(K) + ((size_t)ch * 2 + par) * SB;
+                for (int g = 0; g < 2; g++) {
+                    const int kp = 2 * ch + g;
+                    if (kp >= H) continue;  // padding pair (K = 2): zero rows
+                    for (int jj = 0; jj < H; jj++) {
+                        const int j = 2 * jj + par, t = bf_tw_index(K, fusedN, mid, kp, j);
+                        const int64_t cf[2] = {T.c[t], (int64_t)sign * T.s[t]};
+                        for (int h = 0; h < 2; h++)
+                            for (int i = 0; i < R_MOD; i++) {
+                                const int a = residue_of(cf[h], kModuli[i]);
+                                for (int b = 0; b < 7; b++) {
+                                    const int v = (a * p256[i][b]) % kModuli[i], kap = h * PB + jj * 7 + b;
+                                    for (int d = 0; d < 2; d++) {
+                                        const int n = g * 24 + i * 2 + d;
+                                        dst[(kap / 16) * (BF_N * 16) + n * 16 + kap % 16] = (uint8_t)(d ? v >> 8 : v & 255);
+                                    }
+                                }
+                            }
+                    }
+                }
+            }
+    }
+}
+
+// host: Phase-A constant matrix [kappa/16][n = o*16 + s][16 B], kappa = part*96 + (i*2 + d)*4 + b (part 0 = even-j
+// sum, 1 = odd-j sum): byte s of U = 256^(d+b) u_i mod M, or of M - U for (part 1, o = 1): out_{k+H} = S^E - S^O.
+inline void build_pa_bf(uint8_t *pa, const CrtConsts &C) {
+    for (int i = 0; i < BF_PA_BYTES; i++) pa[i] = 0;
+    for (int i = 0; i < R_MOD; i++) {
+        u128 U = C.u[i] % C.M;
+        for (int e = 0; e < 5; e++) {  // e = d + b
+            for (int d = 0; d < 2; d++) {
+                const int b = e - d;
+                if (b < 0 || b > 3) continue;
+                for (int part = 0; part < 2; part++)
+                    for (int o = 0; o < 2; o++) {
+                        const u128 X = (part && o) ? (C.M - U) % C.M : U;
+                        const int kap = part * 96 + (i * 2 + d) * 4 + b;
+                        for (int s = 0; s < 16; s++)
+                            pa[(kap / 16) * (32 * 16) + (o * 16 + s) * 16 + kap % 16] = (uint8_t)(X >> (8 * s));
+                    }
+            }
+            U = (U << 8) % C.M;
+        }
+    }
+}
+
+
+// ---------------------------------------------------------------------------------------------------- kernel
+// Warp roles (640 threads): warp 0 = matrix producer (TMA bulk copies into a ring), warp 1 = MMA issuer,
+// warps 2-3 idle, warps 4-7 = deconstruction (a1-a3: load, column exponent, quantise, byte planes),
+// warps 8-19 = epilogue (a7-a9, a12: deposits, lift, pack, store; three groups of four warps, one TMEM lane
+// quarter each).  All hand-offs are mbarriers; there is no block-wide barrier inside the tile loop.
+constexpr int BF_THREADS = 640;
+constexpr int BF_NSLOT = 4;         // matrix ring slots (one parity of one chunk each)
+constexpr int BF_DPA = 384;         // TMEM column of the Phase-A results: [slot g][part][o][16 slices]
+template <int K> __host__ __device__ constexpr size_t bf_smem_bytes() {
+    return 2 * (size_t)bf_aset_bytes(K) + (size_t)BF_NSLOT * bf_slot_bytes(K) + BF_PA_BYTES;
+}
+
+// bounded wait: a pipeline bug must not hang the GPU (traps after ~2^28 failed polls, i.e. several seconds)
+__device__ __forceinline__ void bf_wait(uint64_t *bar, uint32_t parity) {
+    const uint32_t a = smem_u32(bar);
+    uint32_t done, spins = 0;
+    do {
+        asm volatile("{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\tselp.u32 %0, 1, 0, p;\n\t}"
+                     : "=r"(done) : "r"(a), "r"(parity) : "memory");
+        if (!done && ++spins > (1u << 28)) __trap();
+    } while (!done);
+}
+
+// append the 7 bytes of w = (hi:lo) (hi < 2^24) at byte position 7 e of a little-endian word array; e is a
+// compile-time constant after unrolling, so every index and shift folds
+__device__ __forceinline__ void bf_append7(uint32_t *wd, int e, uint32_t lo, uint32_t hi) {
+    const int t = (7 * e) / 4, s = ((7 * e) % 4) * 8;
+    if (s == 0) { wd[t] = lo; wd[t + 1] = hi; }
+    else {
+        wd[t] |= lo << s;
+        wd[t + 1] = __funnelshift_l(lo, hi, s);
+        if (s >= 16) wd[t + 2] = hi >> (32 - s);
+    }
+}
+
+template <int K>
+__global__ void __launch_bounds__(BF_THREADS, 1) stage_bf_kernel(StageGeom g, const uint4 *__restrict__ in, uint4 *__restrict__ out,
+                                                                 const uint8_t *__restrict__ mat, const uint4 *__restrict__ ctab,
+                                                                 const uint4 *__restrict__ pa_g, long long ntiles) {
+    constexpr int H = bf_H(K), PB = bf_PB(K), NCK = bf_NCK(K), NCH = bf_NCH(K);
+    constexpr int SB = bf_slot_bytes(K), PLANE = bf_plane_bytes(K), ASET = bf_aset_bytes(K), PARB = NCK * BF_COLS * 16;
+    constexpr int NW = PB / 4;
+    extern __shared__ __align__(128) uint8_t smem[];
+    __shared__ __align__(8) uint64_t a_full[2], a_empty[2], b_full[BF_NSLOT], b_empty[BF_NSLOT], pa_full[3], pa_empty[3];
+    __shared__ uint32_t s_tmem;
+    __shared__ int s_T[2][BF_COLS], s_flag[2][BF_COLS];
+    uint8_t *sA = smem, *sB = smem + 2 * ASET, *sPA = sB + BF_NSLOT * SB;
+
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+    const int lg_nbt = 32 - __clz(((g.nb + 3) >> 2) - 1), lg_ns = 31 - __clz(g.ns);
+
+    for (int i = tid; i < BF_PA_BYTES / 16; i += BF_THREADS) ((uint4 *)sPA)[i] = __ldg(pa_g + i);
+    if (warp == 0) tmem_alloc<512>(&s_tmem);
+    if (tid == 0) {
+        // pa_full / pa_empty are per epilogue group (a waiter must see every phase of its barrier in turn:
+        // try_wait on parity p passes at once while the barrier is still in the phase before p)
+        for (int i = 0; i < 2; i++) { mbar_init(&a_full[i], 8); mbar_init(&a_empty[i], 13); }
+        for (int i = 0; i < 3; i++) { mbar_init(&pa_full[i], 1); mbar_init(&pa_empty[i], 4); }
+        for (int i = 0; i < BF_NSLOT; i++) { mbar_init(&b_full[i], 1); mbar_init(&b_empty[i], 1); }
+        mbar_fence_init();
+    }
+    fence_async_smem();
+    tc_fence_before();
+    __syncthreads();
+    tc_fence_after();
+    const uint32_t tmem = s_tmem;
+
+    if (warp == 0) {
+        // ------------------------------------------------ matrix producer
+        if (lane == 0) {
+            uint32_t m = 0;
+            for (long long tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
+                int tb, ts, to;
+                tile_coords_pow2(g, tile, lg_nbt, lg_ns, tb, ts, to);
+                const uint8_t *mb = mat + (size_t)(g.matsel ? ts : 0) * bf_mat_bytes(K);
+                for (int c = 0; c < 2 * NCH; c++, m++) {
+                    const uint32_t slot = m % BF_NSLOT, use = m / BF_NSLOT;
+                    if (use) bf_wait(&b_empty[slot], (use - 1) & 1);
+                    mbar_expect_tx(&b_full[slot], SB);
+                    bulk_g2s(sB + slot * SB, mb + (size_t)c * SB, SB, &b_full[slot]);
+                }
+            }
+        }
+        __syncwarp();
+    } else if (warp == 1) {
+        // ------------------------------------------------ MMA issuer
+        if (lane == 0) {
+            const uint32_t idesc_st = make_idesc(CFMT_S32, I8_U8, I8_U8, 128, BF_N), idesc_pa = make_idesc(CFMT_S32, I8_U8, I8_U8, 128, 32);
+            const uint32_t sA0 = smem_u32(sA), sB0 = smem_u32(sB), sPA0 = smem_u32(sPA);
+            uint32_t m = 0, n = 0;  // matrix-slot uses, chunks issued
+            auto issue_pa = [&](uint32_t np) {  // Phase A of chunk np (its stage accumulators sit in D buffer np & 1)
+                const uint32_t q = np & 1;
+#pragma unroll
+                for (int gg = 0; gg < 2; gg++) {
+                    const uint32_t u = 2 * np + gg;  // unit index; its D_PA slot gg was last used by unit u - 2
+                    if (u >= 2) bf_wait(&pa_empty[(u - 2) % 3], ((u - 2) / 3) & 1);
+                    tc_fence_after();
+#pragma unroll
+                    for (int P = 0; P < 2; P++)
+#pragma unroll
+                        for (int s = 0; s < 6; s++) {
+                            const uint32_t acol = tmem + q * 192 + P * 96 + (s >= 3 ? 48 : 0) + gg * 24 + (s % 3) * 8;
+                            mma_i8_ts(tmem + BF_DPA + gg * 64 + P * 32, acol, make_sdesc(sPA0 + s * 2 * (32 * 16), 32 * 16, 128), idesc_pa, s > 0);
+                        }
+                    tc_commit(&pa_full[u % 3]);
+                }
+            };
+            uint32_t it = 0;
+            for (long long tile = blockIdx.x; tile < ntiles; tile += gridDim.x, it++) {
+                const uint32_t buf = it & 1;
+                bf_wait(&a_full[buf], (it >> 1) & 1);
+                tc_fence_after();
+                for (int ch = 0; ch < NCH; ch++, n++) {
+                    const uint32_t q = n & 1;
+#pragma unroll
+                    for (int par = 0; par < 2; par++, m++) {
+                        const uint32_t slot = m % BF_NSLOT;
+                        bf_wait(&b_full[slot], (m / BF_NSLOT) & 1);
+                        tc_fence_after();
+#pragma unroll
+                        for (int P = 0; P < 2; P++) {  // P = 0: re rows [XR ; NXI], P = 1: im rows [XI ; XR]
+                            const uint32_t abase = sA0 + buf * ASET + (1 - P) * PLANE + par * PARB;
+#pragma unroll
+                            for (int s = 0; s < NCK; s++) {  // K step s = logical chunks 2s, 2s+1 of [block 0 | block 1]
+                                const int L0 = 2 * s, L1 = 2 * s + 1;
+                                const uint32_t a0 = abase + (L0 / NCK) * PLANE + (L0 % NCK) * (BF_COLS * 16);
+                                const uint32_t a1 = abase + (L1 / NCK) * PLANE + (L1 % NCK) * (BF_COLS * 16);
+                                mma_i8_ss(tmem + q * 192 + P * 96 + par * 48, make_sdesc(a0, a1 - a0, 128),
+                                          make_sdesc(sB0 + slot * SB + s * 2 * (BF_N * 16), BF_N * 16, 128), idesc_st, s > 0);
+                            }
+                        }
+                        tc_commit(&b_empty[slot]);
+                    }
+                    if (ch == NCH - 1) tc_commit(&a_empty[buf]);
+                    if (n) issue_pa(n - 1);  // one chunk behind, so the tensor pipe always has stage work queued
+                }
+            }
+            if (n) issue_pa(n - 1);
+        }
+        __syncwarp();
+    } else if (warp >= 4 && warp < 8) {
+        // ------------------------------------------------ deconstruction: thread = (column, parity of j)
+        const int dw = warp - 4, par = lane >> 4;
+        uint32_t it = 0;
+        for (long long tile = blockIdx.x; tile < ntiles; tile += gridDim.x, it++) {
+            const uint32_t buf = it & 1;
+            int tb, ts, to;
+            tile_coords_pow2(g, tile, lg_nbt, lg_ns, tb, ts, to);
+            if (it >= 2) bf_wait(&a_empty[buf], ((it >> 1) - 1) & 1);
+#pragma unroll 1
+            for (int hh = 0; hh < 2; hh++) {
+                const int c = hh * 64 + dw * 16 + (lane & 15);
+                const int blk = 4 * tb + (c >> 5);
+                const bool valid = blk < g.nb;
+                const uint4 *src = in + ((long long)blk * g.ib + (long long)ts * g.is + (long long)to * g.io + (long long)(c & 31) * g.lane + (long long)par * g.ji);
+                const long long jstep = 2 * g.ji;
+                // a2: column exponent = max of the 11-bit exponent fields (integer compare on the high words)
+                uint32_t hmax = 0;
+#pragma unroll
+                for (int jj = 0; jj < H; jj++) {
+                    const uint4 v = valid ? __ldg(src + jj * jstep) : make_uint4(0, 0, 0, 0);
+                    hmax = max(hmax, max(v.y & 0x7FFFFFFFu, v.w & 0x7FFFFFFFu));
+                }
+                hmax = max(hmax, __shfl_xor_sync(0xFFFFFFFFu, hmax, 16));
+                int Tmax = 0, flag = 0;
+                const uint32_t ef = hmax >> 20;
+                if (ef == 0x7FF) flag = 2;
+                else if (ef) { flag = 1; Tmax = (int)ef - 1023; }
+                if (__any_sync(0xFFFFFFFFu, ef == 0)) {  // some column holds only zeros and subnormals: true leading bits
+                    int tm = -100000;                   // (warp-uniform branch: the exchange below needs every lane)
+                    for (int jj = 0; jj < H; jj++) {
+                        const uint4 v = valid ? __ldg(src + jj * jstep) : make_uint4(0, 0, 0, 0);
+                        int T;
+                        if (classify_top(((uint64_t)v.y << 32) | v.x, T) == CLS_FINITE) tm = max(tm, T);
+                        if (classify_top(((uint64_t)v.w << 32) | v.z, T) == CLS_FINITE) tm = max(tm, T);
+                    }
+                    tm = max(tm, __shfl_xor_sync(0xFFFFFFFFu, tm, 16));
+                    if (ef == 0 && tm > -100000) { flag = 1; Tmax = tm; }
+                }
+                if (par == 0) { s_T[buf][c] = Tmax; s_flag[buf][c] = flag; }
+                // a3: quantise, offset by 2^53, split into bytes; planes XI (0), XR (1), NXI (2)
+                uint32_t wr[NW + 2], wi[NW + 2], wn[NW + 2];
+#pragma unroll
+                for (int t = 0; t < NW + 2; t++) wr[t] = wi[t] = wn[t] = 0;
+                uint8_t *dst = sA + buf * ASET + par * PARB + c * 16;
+#pragma unroll
+                for (int e = 0; e < H; e++) {
+                    const uint4 v = valid ? __ldg(src + e * jstep) : make_uint4(0, 0, 0, 0);
+                    const uint64_t br = ((uint64_t)v.y << 32) | v.x, bi = ((uint64_t)v.w << 32) | v.z;
+                    const uint64_t ar = flag == 1 ? quantise_mag_fast(br, Tmax) : 0ull, ai = flag == 1 ? quantise_mag_fast(bi, Tmax) : 0ull;
+                    const uint64_t sr = (uint64_t)((int64_t)br >> 63), si = (uint64_t)((int64_t)bi >> 63);
+                    const uint64_t off = 1ull << 53;
+                    const uint64_t qr = ((ar ^ sr) - sr) + off, qi = ((ai ^ si) - si) + off, qn = 2 * off - qi;
+                    bf_append7(wr, e, (uint32_t)qr, (uint32_t)(qr >> 32));
+                    bf_append7(wi, e, (uint32_t)qi, (uint32_t)(qi >> 32));
+                    bf_append7(wn, e, (uint32_t)qn, (uint32_t)(qn >> 32));
+#pragma unroll
+                    for (int t = 0; t < NCK; t++)
+                        if (16 * (t + 1) <= 7 * (e + 1) && 16 * (t + 1) > 7 * e) {  // chunk t just completed
+                            *(uint4 *)(dst + t * (BF_COLS * 16)) = make_uint4(wi[4 * t], wi[4 * t + 1], wi[4 * t + 2], wi[4 * t + 3]);
+                            *(uint4 *)(dst + PLANE + t * (BF_COLS * 16)) = make_uint4(wr[4 * t], wr[4 * t + 1], wr[4 * t + 2], wr[4 * t + 3]);
+                            *(uint4 *)(dst + 2 * PLANE + t * (BF_COLS * 16)) = make_uint4(wn[4 * t], wn[4 * t + 1], wn[4 * t + 2], wn[4 * t + 3]);
+                        }
+                }
+#pragma unroll
+                for (int t = 0; t < NCK; t++)
+                    if (16 * (t + 1) > 7 * H) {  // trailing chunk(s) that the last element did not complete (zero padded)
+                        *(uint4 *)(dst + t * (BF_COLS * 16)) = make_uint4(wi[4 * t], wi[4 * t + 1], wi[4 * t + 2], wi[4 * t + 3]);
+                        *(uint4 *)(dst + PLANE + t * (BF_COLS * 16)) = make_uint4(wr[4 * t], wr[4 * t + 1], wr[4 * t + 2], wr[4 * t + 3]);
+                        *(uint4 *)(dst + 2 * PLANE + t * (BF_COLS * 16)) = make_uint4(wn[4 * t], wn[4 * t + 1], wn[4 * t + 2], wn[4 * t + 3]);
+                    }
+                fence_async_smem();
+                __syncwarp();
+                if (lane == 0) mbar_arrive(&a_full[buf]);
+            }
+        }
+    } else if (warp >= 8) {
+        // ------------------------------------------------ epilogue: thread = data column (TMEM lane), both parts
+        const int qd = (warp - 8) >> 2, row = (warp & 3) * 32 + lane;
+        const uint32_t lane_taddr = tmem + ((uint32_t)((warp & 3) * 32) << 16);
+        uint32_t it = 0, u = 0;
+        for (long long tile = blockIdx.x; tile < ntiles; tile += gridDim.x, it++) {
+            const uint32_t buf = it & 1;
+            int tb, ts, to;
+            tile_coords_pow2(g, tile, lg_nbt, lg_ns, tb, ts, to);
+            const int blk = 4 * tb + (row >> 5);
+            const bool valid = blk < g.nb;
+            uint4 *dstp = out + ((long long)blk * g.ob + (long long)ts * g.os + (long long)to * g.oo + (long long)(row & 31) * g.lane);
+            const uint4 *ct = ctab + (size_t)(g.matsel ? ts : 0) * K;
+            bf_wait(&a_full[buf], (it >> 1) & 1);
+            const int Tmax = s_T[buf][row], flag = s_flag[buf][row];
+            __syncwarp();
+            if (lane == 0) mbar_arrive(&a_empty[buf]);
+            const int gexp = 53 + 52 - Tmax;
+#pragma unroll 1
+            for (int ch = 0; ch < NCH; ch++)
+#pragma unroll 1
+                for (int gg = 0; gg < 2; gg++, u++) {
+                    if ((int)(u % 3) != qd) continue;
+                    bf_wait(&pa_full[qd], (u / 3) & 1);
+                    tc_fence_after();
+                    uint32_t E[4][5];  // [part*2 + o]
+#pragma unroll
+                    for (int x = 0; x < 4; x++) {
+                        uint32_t P[16];
+                        tmem_ld_x16(lane_taddr + BF_DPA + gg * 64 + x * 16, P);
+                        tmem_ld_wait();
+                        slices_to_E(P, E[x]);
+                    }
+                    tc_fence_before();
+                    __syncwarp();
+                    if (lane == 0) mbar_arrive(&pa_empty[qd]);
+                    const int kp = 2 * ch + gg;
+                    if (kp >= H) continue;
+#pragma unroll
+                    for (int o = 0; o < 2; o++) {
+                        const int k = kp + o * H;
+                        const uint4 cc = __ldg(ct + k);
+                        uint64_t y[2];
+#pragma unroll
+                        for (int P = 0; P < 2; P++) {
+                            if (flag & 2) y[P] = 0x7FF8000000000000ull;
+                            else if (flag == 0) y[P] = 0;
+                            else {
+                                const uint32_t *e = E[P * 2 + o];
+                                uint32_t r[4], r2[4];
+                                crt_from_E(e[0], e[1], e[2], e[3], e[4], r);
+                                sub128(r2, r[0], r[1], r[2], r[3], cc.x, cc.y, cc.z, cc.w);
+                                y[P] = pack_limbs(r2, gexp);
+                            }
+                        }
+                        if (valid) dstp[(long long)k * g.ko] = make_uint4((uint32_t)y[0], (uint32_t)(y[0] >> 32), (uint32_t)y[1], (uint32_t)(y[1] >> 32));
+                    }
+                }
+        }
+    }
+    tc_fence_before();
+    __syncthreads();
+    if (warp == 0) tmem_dealloc<512>(tmem);
+}
+
+template <int K>
+inline bool stage_bf_launch_k(const StageGeom &g, const void *in, void *out, const uint8_t *mat, const void *ctab, const void *pa,
+                              long long nt, int sms, cudaStream_t st) {
+    const unsigned grid = (unsigned)(nt < sms ? nt : sms);
+    stage_bf_kernel<K><<<grid, BF_THREADS, bf_smem_bytes<K>(), st>>>(g, (const uint4 *)in, (uint4 *)out, mat, (const uint4 *)ctab, (const uint4 *)pa, nt);
+    return cudaGetLastError() == cudaSuccess;
+}
+
+inline bool stage_bf_prepare() {
+    cudaError_t e = cudaFuncSetAttribute(stage_bf_kernel<32>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bf_smem_bytes<32>());
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(stage_bf_kernel<16>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bf_smem_bytes<16>());
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(stage_bf_kernel<8>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bf_smem_bytes<8>());
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(stage_bf_kernel<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bf_smem_bytes<4>());
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(stage_bf_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bf_smem_bytes<2>());
+    return e == cudaSuccess;
+}
+
+// tiles of 128 columns = 4 blocks of 32; the block grid along b is rounded up to a power of two (masked surplus)
+inline bool stage_bf_launch(const StageGeom &g, const void *src, void *dst, const uint8_t *mat, const void *ctab, const void *pa, int sms,
+                            cudaStream_t st) {
+    int nbt = 1;
+    while (nbt < (g.nb + 3) / 4) nbt <<= 1;
+    if (g.ns & (g.ns - 1)) return false;
+    const long long nt = (long long)nbt * g.ns * g.no;
+    if (nt >= (1ll << 31)) return false;
+    switch (g.K) {
+        case 32: return stage_bf_launch_k<32>(g, src, dst, mat, ctab, pa, nt, sms, st);
+        case 16: return stage_bf_launch_k<16>(g, src, dst, mat, ctab, pa, nt, sms, st);
+        case 8: return stage_bf_launch_k<8>(g, src, dst, mat, ctab, pa, nt, sms, st);
+        case 4: return stage_bf_launch_k<4>(g, src, dst, mat, ctab, pa, nt, sms, st);
+        case 2: return stage_bf_launch_k<2>(g, src, dst, mat, ctab, pa, nt, sms, st);
+    }
+    return false;
+}
+
+}  // namespace oz

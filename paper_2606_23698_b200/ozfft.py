@@ -12,7 +12,7 @@ _lib = None
 
 SYMBOLS = ["ozfft_plan_create", "ozfft_plan_create_1d", "ozfft_exec", "ozfft_exec_host", "ozfft_plan_destroy",
            "ozfft_last_error", "ozfft_twiddle_checksum", "ozfft_plan_num_launches", "ozfft_plan_device_bytes",
-           "ozfft_exec_axis", "ozfft_probe_mma", "ozfft_probe_chain", "ozfft_probe_crt"]
+           "ozfft_exec_axis", "ozfft_probe_mma", "ozfft_probe_chain", "ozfft_probe_crt", "ozfft_debug_bf_tables"]
 
 
 def lib():
@@ -39,6 +39,8 @@ def lib():
         L.ozfft_probe_mma.argtypes = [C.c_int, C.c_int, C.c_int, vp, vp, vp, vp]
         L.ozfft_probe_chain.argtypes = [C.c_int, C.c_int, C.c_int, vp, vp, vp, vp, vp, vp]
         L.ozfft_probe_crt.argtypes = [C.c_int, vp, vp, C.c_int, vp]
+        L.ozfft_debug_bf_tables.restype = C.c_size_t
+        L.ozfft_debug_bf_tables.argtypes = [C.c_int, C.c_int, C.c_int, vp, vp, vp]
         _lib = L
     return _lib
 
@@ -156,3 +158,17 @@ def probe_crt(residues, variant):
     out = torch.zeros((n, 4), dtype=torch.int32, device=residues.device)
     _check(lib().ozfft_probe_crt(n, residues.data_ptr(), out.data_ptr(), variant, _stream(None)), "ozfft_probe_crt")
     return out
+
+
+def debug_bf_tables(K, fusedN, sign):
+    """Host tables of the byte-fed stage kernel as numpy arrays (B planes uint8, C limbs uint32 [nmat*K, 4], PA uint8)."""
+    import numpy as np
+    size = lib().ozfft_debug_bf_tables(K, fusedN, sign, None, None, None)
+    if not size:
+        raise ValueError("bad (K, fusedN, sign)")
+    nmat = 32 if fusedN else 1
+    B = np.zeros(size, dtype=np.uint8)
+    Cc = np.zeros((nmat * K, 4), dtype=np.uint32)
+    PA = np.zeros(6144, dtype=np.uint8)
+    lib().ozfft_debug_bf_tables(K, fusedN, sign, B.ctypes.data, Cc.ctypes.data, PA.ctypes.data)
+    return B, Cc, PA

@@ -8,9 +8,10 @@ pytestmark = pytest.mark.gpu
 TOL_F128 = 5e-15  # north_star: normwise relative error vs the __float128 naive DFT
 
 
-@pytest.fixture(autouse=True, params=["tc", "simt"])
+@pytest.fixture(autouse=True, params=["bf", "tc", "simt"])
 def variant(request, monkeypatch):
-    """every parity case runs on the tensor-core kernel and on the all-SIMT cross-check kernel"""
+    """every parity case runs on the byte-fed tensor-core kernel (the default), on the residue-digit tensor-core
+    kernel and on the all-SIMT cross-check kernel"""
     monkeypatch.setenv("OZFFT_VARIANT", request.param)
     return request.param
 
@@ -168,7 +169,7 @@ def test_bad_arguments():
 def test_exec_host_pipelined_path(O, variant):
     """sizes >= 2^24 elements take the slab pipeline in ozfft_exec_host (copies overlapped with the passes):
     same bits as the device-resident call and as the oracle"""
-    if variant != "tc":
+    if variant != "bf":
         pytest.skip("pipeline logic is kernel-independent; run once")
     torch = _torch()
     from paper_2606_23698_b200 import inputs, ozfft
