@@ -278,7 +278,7 @@ def run_ours(args):
             "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "int32", "data": "synthetic",
             "config": {"workload": f"forward 3-D FFT {size}^3 complex128, uniform[-1,1), seed {SEED} (BASELINE.json configs[4])",
                        "parallelism": "replicas only" if world > 1 else "single GPU", "l2": "inputs_exceed_l2" if nbytes > (126 << 20) else "l2_resident",
-                       "variant": os.environ.get("OZFFT_VARIANT", "tc"), "stage_launches_per_transform": launches},
+                       "variant": os.environ.get("OZFFT_VARIANT", "bf"), "stage_launches_per_transform": launches},
             "ms_per_transform": ms_step_max, "ms_per_transform_min": min(ms), "inverse_ms": inv_ms,
             "roundtrip_rel_err": roundtrip, "host_and_device_paths_bit_identical": same,
             "hbm_roof": {"alg_bytes": 96.0 * n_tot if launches == 6 else alg_bytes_launch * launches / 2,

@@ -125,11 +125,11 @@ inline void build_pa_bf(uint8_t *pa, const CrtConsts &C) {
 
 
 // ---------------------------------------------------------------------------------------------------- kernel
-// Warp roles (640 threads): warp 0 = matrix producer (TMA bulk copies into a ring), warp 1 = MMA issuer,
-// warps 2-3 idle, warps 4-7 = deconstruction (a1-a3: load, column exponent, quantise, byte planes),
-// warps 8-19 = epilogue (a7-a9, a12: deposits, lift, pack, store; three groups of four warps, one TMEM lane
+// Warp roles (768 threads): warp 0 = matrix producer (TMA bulk copies into a ring), warp 1 = stage MMA issuer,
+// warp 2 = Phase-A MMA issuer, warp 3 idle, warps 4-11 = deconstruction (a1-a3: load, column exponent, quantise, byte planes),
+// warps 12-23 = epilogue (a7-a9, a12: deposits, lift, pack, store; three groups of four warps, one TMEM lane
 // quarter each).  All hand-offs are mbarriers; there is no block-wide barrier inside the tile loop.
-constexpr int BF_THREADS = 640;
+constexpr int BF_THREADS = 768;
 constexpr int BF_NSLOT = 4;         // matrix ring slots (one parity of one chunk each)
 constexpr int BF_DPA = 384;         // TMEM column of the Phase-A results: [slot g][part][o][16 slices]
 template <int K> __host__ __device__ constexpr size_t bf_smem_bytes() {
@@ -167,7 +167,7 @@ __global__ void __launch_bounds__(BF_THREADS, 1) stage_bf_kernel(StageGeom g, co
     constexpr int SB = bf_slot_bytes(K), PLANE = bf_plane_bytes(K), ASET = bf_aset_bytes(K), PARB = NCK * BF_COLS * 16;
     constexpr int NW = PB / 4;
     extern __shared__ __align__(128) uint8_t smem[];
-    __shared__ __align__(8) uint64_t a_full[2], a_empty[2], b_full[BF_NSLOT], b_empty[BF_NSLOT], pa_full[3], pa_empty[3];
+    __shared__ __align__(8) uint64_t a_full[2], a_empty[2], b_full[BF_NSLOT], b_empty[BF_NSLOT], pa_full[3], pa_empty[3], st_done[2], d_free[2];
     __shared__ uint32_t s_tmem;
     __shared__ int s_T[2][BF_COLS], s_flag[2][BF_COLS];
     uint8_t *sA = smem, *sB = smem + 2 * ASET, *sPA = sB + BF_NSLOT * SB;
@@ -180,7 +180,7 @@ __global__ void __launch_bounds__(BF_THREADS, 1) stage_bf_kernel(StageGeom g, co
     if (tid == 0) {
         // pa_full / pa_empty are per epilogue group (a waiter must see every phase of its barrier in turn:
         // try_wait on parity p passes at once while the barrier is still in the phase before p)
-        for (int i = 0; i < 2; i++) { mbar_init(&a_full[i], 8); mbar_init(&a_empty[i], 13); }
+        for (int i = 0; i < 2; i++) { mbar_init(&a_full[i], 8); mbar_init(&a_empty[i], 13); mbar_init(&st_done[i], 1); mbar_init(&d_free[i], 1); }
         for (int i = 0; i < 3; i++) { mbar_init(&pa_full[i], 1); mbar_init(&pa_empty[i], 4); }
         for (int i = 0; i < BF_NSLOT; i++) { mbar_init(&b_full[i], 1); mbar_init(&b_empty[i], 1); }
         mbar_fence_init();
@@ -192,126 +192,143 @@ __global__ void __launch_bounds__(BF_THREADS, 1) stage_bf_kernel(StageGeom g, co
     const uint32_t tmem = s_tmem;
 
     if (warp == 0) {
-        // ------------------------------------------------ matrix producer
-        if (lane == 0) {
-            uint32_t m = 0;
-            for (long long tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
-                int tb, ts, to;
-                tile_coords_pow2(g, tile, lg_nbt, lg_ns, tb, ts, to);
-                const uint8_t *mb = mat + (size_t)(g.matsel ? ts : 0) * bf_mat_bytes(K);
-                for (int c = 0; c < 2 * NCH; c++, m++) {
-                    const uint32_t slot = m % BF_NSLOT, use = m / BF_NSLOT;
-                    if (use) bf_wait(&b_empty[slot], (use - 1) & 1);
+        // ------------------------------------------------ matrix producer (whole warp walks the loop, one lane issues)
+        uint32_t m = 0;
+        for (long long tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
+            int tb, ts, to;
+            tile_coords_pow2(g, tile, lg_nbt, lg_ns, tb, ts, to);
+            const uint8_t *mb = mat + (size_t)(g.matsel ? ts : 0) * bf_mat_bytes(K);
+            for (int c = 0; c < 2 * NCH; c++, m++) {
+                const uint32_t slot = m % BF_NSLOT, use = m / BF_NSLOT;
+                if (use) bf_wait(&b_empty[slot], (use - 1) & 1);
+                if (elect_one()) {
                     mbar_expect_tx(&b_full[slot], SB);
                     bulk_g2s(sB + slot * SB, mb + (size_t)c * SB, SB, &b_full[slot]);
                 }
+                __syncwarp();
             }
         }
-        __syncwarp();
     } else if (warp == 1) {
-        // ------------------------------------------------ MMA issuer
-        if (lane == 0) {
-            const uint32_t idesc_st = make_idesc(CFMT_S32, I8_U8, I8_U8, 128, BF_N), idesc_pa = make_idesc(CFMT_S32, I8_U8, I8_U8, 128, 32);
-            const uint32_t sA0 = smem_u32(sA), sB0 = smem_u32(sB), sPA0 = smem_u32(sPA);
-            uint32_t m = 0, n = 0;  // matrix-slot uses, chunks issued
-            auto issue_pa = [&](uint32_t np) {  // Phase A of chunk np (its stage accumulators sit in D buffer np & 1)
-                const uint32_t q = np & 1;
+        // ------------------------------------------------ stage MMA issuer: a4 (with a3 and a5 folded into the operands)
+        // every descriptor is one base plus a compile-time constant (address in 16-byte units in bits 0-13, the
+        // leading-dimension byte offset in bits 16-29)
+        const uint32_t idesc_st = make_idesc(CFMT_S32, I8_U8, I8_U8, 128, BF_N);
+        const uint64_t bdesc0 = make_sdesc(smem_u32(sB), BF_N * 16, 128);
+        uint32_t m = 0, n = 0, it = 0;
+        for (long long tile = blockIdx.x; tile < ntiles; tile += gridDim.x, it++) {
+            const uint32_t buf = it & 1;
+            bf_wait(&a_full[buf], (it >> 1) & 1);
+            const uint64_t adesc0 = make_sdesc(smem_u32(sA) + buf * ASET, BF_COLS * 16, 128);
+            for (int ch = 0; ch < NCH; ch++, n++) {
+                const uint32_t q = n & 1;
+                if (n >= 2) bf_wait(&d_free[q], ((n >> 1) - 1) & 1);  // Phase A of chunk n-2 has read this accumulator buffer
 #pragma unroll
-                for (int gg = 0; gg < 2; gg++) {
-                    const uint32_t u = 2 * np + gg;  // unit index; its D_PA slot gg was last used by unit u - 2
-                    if (u >= 2) bf_wait(&pa_empty[(u - 2) % 3], ((u - 2) / 3) & 1);
+                for (int par = 0; par < 2; par++, m++) {
+                    const uint32_t slot = m % BF_NSLOT;
+                    bf_wait(&b_full[slot], (m / BF_NSLOT) & 1);
                     tc_fence_after();
+                    if (elect_one()) {
+                        const uint64_t bd = bdesc0 + (uint64_t)((slot * SB) >> 4);
 #pragma unroll
-                    for (int P = 0; P < 2; P++)
-#pragma unroll
-                        for (int s = 0; s < 6; s++) {
-                            const uint32_t acol = tmem + q * 192 + P * 96 + (s >= 3 ? 48 : 0) + gg * 24 + (s % 3) * 8;
-                            mma_i8_ts(tmem + BF_DPA + gg * 64 + P * 32, acol, make_sdesc(sPA0 + s * 2 * (32 * 16), 32 * 16, 128), idesc_pa, s > 0);
-                        }
-                    tc_commit(&pa_full[u % 3]);
-                }
-            };
-            uint32_t it = 0;
-            for (long long tile = blockIdx.x; tile < ntiles; tile += gridDim.x, it++) {
-                const uint32_t buf = it & 1;
-                bf_wait(&a_full[buf], (it >> 1) & 1);
-                tc_fence_after();
-                for (int ch = 0; ch < NCH; ch++, n++) {
-                    const uint32_t q = n & 1;
-#pragma unroll
-                    for (int par = 0; par < 2; par++, m++) {
-                        const uint32_t slot = m % BF_NSLOT;
-                        bf_wait(&b_full[slot], (m / BF_NSLOT) & 1);
-                        tc_fence_after();
-#pragma unroll
-                        for (int P = 0; P < 2; P++) {  // P = 0: re rows [XR ; NXI], P = 1: im rows [XI ; XR]
-                            const uint32_t abase = sA0 + buf * ASET + (1 - P) * PLANE + par * PARB;
+                        for (int P = 0; P < 2; P++)  // P = 0: re rows [XR ; NXI], P = 1: im rows [XI ; XR]
 #pragma unroll
                             for (int s = 0; s < NCK; s++) {  // K step s = logical chunks 2s, 2s+1 of [block 0 | block 1]
                                 const int L0 = 2 * s, L1 = 2 * s + 1;
-                                const uint32_t a0 = abase + (L0 / NCK) * PLANE + (L0 % NCK) * (BF_COLS * 16);
-                                const uint32_t a1 = abase + (L1 / NCK) * PLANE + (L1 % NCK) * (BF_COLS * 16);
-                                mma_i8_ss(tmem + q * 192 + P * 96 + par * 48, make_sdesc(a0, a1 - a0, 128),
-                                          make_sdesc(sB0 + slot * SB + s * 2 * (BF_N * 16), BF_N * 16, 128), idesc_st, s > 0);
+                                const int o0 = (1 - P) * PLANE + par * PARB + (L0 / NCK) * PLANE + (L0 % NCK) * (BF_COLS * 16);
+                                const int o1 = (1 - P) * PLANE + par * PARB + (L1 / NCK) * PLANE + (L1 % NCK) * (BF_COLS * 16);
+                                const uint64_t acon = (uint64_t)(o0 >> 4) + ((uint64_t)((o1 - o0 - BF_COLS * 16) >> 4) << 16);
+                                mma_i8_ss(tmem + q * 192 + P * 96 + par * 48, adesc0 + acon, bd + (uint64_t)((s * 2 * BF_N * 16) >> 4), idesc_st, s > 0);
                             }
-                        }
                         tc_commit(&b_empty[slot]);
+                        if (par == 1) {
+                            tc_commit(&st_done[q]);
+                            if (ch == NCH - 1) tc_commit(&a_empty[buf]);
+                        }
                     }
-                    if (ch == NCH - 1) tc_commit(&a_empty[buf]);
-                    if (n) issue_pa(n - 1);  // one chunk behind, so the tensor pipe always has stage work queued
+                    __syncwarp();
                 }
             }
-            if (n) issue_pa(n - 1);
         }
-        __syncwarp();
-    } else if (warp >= 4 && warp < 8) {
+    } else if (warp == 2) {
+        // ------------------------------------------------ Phase-A MMA issuer: a6, A operand = the stage accumulators in TMEM
+        const uint32_t idesc_pa = make_idesc(CFMT_S32, I8_U8, I8_U8, 128, 32);
+        const uint64_t pdesc0 = make_sdesc(smem_u32(sPA), 32 * 16, 128);
+        uint32_t n = 0;
+        for (long long tile = blockIdx.x; tile < ntiles; tile += gridDim.x)
+            for (int ch = 0; ch < NCH; ch++, n++) {
+                const uint32_t q = n & 1;
+                bf_wait(&st_done[q], (n >> 1) & 1);
+#pragma unroll
+                for (int gg = 0; gg < 2; gg++) {
+                    const uint32_t u = 2 * n + gg;  // unit index; its D_PA slot gg was last used by unit u - 2
+                    if (u >= 2) bf_wait(&pa_empty[(u - 2) % 3], ((u - 2) / 3) & 1);
+                    tc_fence_after();
+                    if (elect_one()) {
+#pragma unroll
+                        for (int P = 0; P < 2; P++)
+#pragma unroll
+                            for (int s = 0; s < 6; s++)
+                                mma_i8_ts(tmem + BF_DPA + gg * 64 + P * 32, tmem + q * 192 + P * 96 + (s >= 3 ? 48 : 0) + gg * 24 + (s % 3) * 8,
+                                          pdesc0 + (uint64_t)((s * 2 * 32 * 16) >> 4), idesc_pa, s > 0);
+                        tc_commit(&pa_full[u % 3]);
+                        if (gg == 1) tc_commit(&d_free[q]);
+                    }
+                    __syncwarp();
+                }
+            }
+    } else if (warp >= 4 && warp < 12) {
         // ------------------------------------------------ deconstruction: thread = (column, parity of j)
-        const int dw = warp - 4, par = lane >> 4;
+        const int dw = warp - 4, par = lane >> 4, c = dw * 16 + (lane & 15);
+        constexpr int BS = H < 8 ? H : 8;  // elements loaded together (memory-level parallelism)
         uint32_t it = 0;
         for (long long tile = blockIdx.x; tile < ntiles; tile += gridDim.x, it++) {
             const uint32_t buf = it & 1;
             int tb, ts, to;
             tile_coords_pow2(g, tile, lg_nbt, lg_ns, tb, ts, to);
-            if (it >= 2) bf_wait(&a_empty[buf], ((it >> 1) - 1) & 1);
-#pragma unroll 1
-            for (int hh = 0; hh < 2; hh++) {
-                const int c = hh * 64 + dw * 16 + (lane & 15);
-                const int blk = 4 * tb + (c >> 5);
-                const bool valid = blk < g.nb;
-                const uint4 *src = in + ((long long)blk * g.ib + (long long)ts * g.is + (long long)to * g.io + (long long)(c & 31) * g.lane + (long long)par * g.ji);
-                const long long jstep = 2 * g.ji;
-                // a2: column exponent = max of the 11-bit exponent fields (integer compare on the high words)
-                uint32_t hmax = 0;
+            const int blk = 4 * tb + (c >> 5);
+            const bool valid = blk < g.nb;
+            const uint4 *src = in + ((long long)blk * g.ib + (long long)ts * g.is + (long long)to * g.io + (long long)(c & 31) * g.lane + (long long)par * g.ji);
+            const long long jstep = 2 * g.ji;
+            // a2: column exponent = max of the 11-bit exponent fields (integer compare on the high words)
+            uint32_t hmax = 0;
 #pragma unroll
+            for (int jj = 0; jj < H; jj++) {
+                const uint4 v = valid ? __ldg(src + jj * jstep) : make_uint4(0, 0, 0, 0);
+                hmax = max(hmax, max(v.y & 0x7FFFFFFFu, v.w & 0x7FFFFFFFu));
+            }
+            hmax = max(hmax, __shfl_xor_sync(0xFFFFFFFFu, hmax, 16));
+            int Tmax = 0, flag = 0;
+            const uint32_t ef = hmax >> 20;
+            if (ef == 0x7FF) flag = 2;
+            else if (ef) { flag = 1; Tmax = (int)ef - 1023; }
+            if (__any_sync(0xFFFFFFFFu, ef == 0)) {  // some column holds only zeros and subnormals: true leading bits
+                int tm = -100000;                   // (warp-uniform branch: the exchange below needs every lane)
                 for (int jj = 0; jj < H; jj++) {
                     const uint4 v = valid ? __ldg(src + jj * jstep) : make_uint4(0, 0, 0, 0);
-                    hmax = max(hmax, max(v.y & 0x7FFFFFFFu, v.w & 0x7FFFFFFFu));
+                    int T;
+                    if (classify_top(((uint64_t)v.y << 32) | v.x, T) == CLS_FINITE) tm = max(tm, T);
+                    if (classify_top(((uint64_t)v.w << 32) | v.z, T) == CLS_FINITE) tm = max(tm, T);
                 }
-                hmax = max(hmax, __shfl_xor_sync(0xFFFFFFFFu, hmax, 16));
-                int Tmax = 0, flag = 0;
-                const uint32_t ef = hmax >> 20;
-                if (ef == 0x7FF) flag = 2;
-                else if (ef) { flag = 1; Tmax = (int)ef - 1023; }
-                if (__any_sync(0xFFFFFFFFu, ef == 0)) {  // some column holds only zeros and subnormals: true leading bits
-                    int tm = -100000;                   // (warp-uniform branch: the exchange below needs every lane)
-                    for (int jj = 0; jj < H; jj++) {
-                        const uint4 v = valid ? __ldg(src + jj * jstep) : make_uint4(0, 0, 0, 0);
-                        int T;
-                        if (classify_top(((uint64_t)v.y << 32) | v.x, T) == CLS_FINITE) tm = max(tm, T);
-                        if (classify_top(((uint64_t)v.w << 32) | v.z, T) == CLS_FINITE) tm = max(tm, T);
-                    }
-                    tm = max(tm, __shfl_xor_sync(0xFFFFFFFFu, tm, 16));
-                    if (ef == 0 && tm > -100000) { flag = 1; Tmax = tm; }
-                }
-                if (par == 0) { s_T[buf][c] = Tmax; s_flag[buf][c] = flag; }
-                // a3: quantise, offset by 2^53, split into bytes; planes XI (0), XR (1), NXI (2)
-                uint32_t wr[NW + 2], wi[NW + 2], wn[NW + 2];
+                tm = max(tm, __shfl_xor_sync(0xFFFFFFFFu, tm, 16));
+                if (ef == 0 && tm > -100000) { flag = 1; Tmax = tm; }
+            }
+            // the previous user of this operand buffer (the stage MMAs of tile it-2) must be done before the writes
+            if (it >= 2) bf_wait(&a_empty[buf], ((it >> 1) - 1) & 1);
+            if (par == 0) { s_T[buf][c] = Tmax; s_flag[buf][c] = flag; }
+            // a3: quantise, offset by 2^53, split into bytes; planes XI (0), XR (1), NXI (2)
+            uint32_t wr[NW + 2], wi[NW + 2], wn[NW + 2];
 #pragma unroll
-                for (int t = 0; t < NW + 2; t++) wr[t] = wi[t] = wn[t] = 0;
-                uint8_t *dst = sA + buf * ASET + par * PARB + c * 16;
+            for (int t = 0; t < NW + 2; t++) wr[t] = wi[t] = wn[t] = 0;
+            uint8_t *dst = sA + buf * ASET + par * PARB + c * 16;
 #pragma unroll
-                for (int e = 0; e < H; e++) {
-                    const uint4 v = valid ? __ldg(src + e * jstep) : make_uint4(0, 0, 0, 0);
+            for (int e0 = 0; e0 < H; e0 += BS) {
+                uint4 vv[BS];
+#pragma unroll
+                for (int x = 0; x < BS; x++) vv[x] = valid ? __ldg(src + (e0 + x) * jstep) : make_uint4(0, 0, 0, 0);
+#pragma unroll
+                for (int x = 0; x < BS; x++) {
+                    const int e = e0 + x;
+                    const uint4 v = vv[x];
                     const uint64_t br = ((uint64_t)v.y << 32) | v.x, bi = ((uint64_t)v.w << 32) | v.z;
                     const uint64_t ar = flag == 1 ? quantise_mag_fast(br, Tmax) : 0ull, ai = flag == 1 ? quantise_mag_fast(bi, Tmax) : 0ull;
                     const uint64_t sr = (uint64_t)((int64_t)br >> 63), si = (uint64_t)((int64_t)bi >> 63);
@@ -328,21 +345,21 @@ __global__ void __launch_bounds__(BF_THREADS, 1) stage_bf_kernel(StageGeom g, co
                             *(uint4 *)(dst + 2 * PLANE + t * (BF_COLS * 16)) = make_uint4(wn[4 * t], wn[4 * t + 1], wn[4 * t + 2], wn[4 * t + 3]);
                         }
                 }
-#pragma unroll
-                for (int t = 0; t < NCK; t++)
-                    if (16 * (t + 1) > 7 * H) {  // trailing chunk(s) that the last element did not complete (zero padded)
-                        *(uint4 *)(dst + t * (BF_COLS * 16)) = make_uint4(wi[4 * t], wi[4 * t + 1], wi[4 * t + 2], wi[4 * t + 3]);
-                        *(uint4 *)(dst + PLANE + t * (BF_COLS * 16)) = make_uint4(wr[4 * t], wr[4 * t + 1], wr[4 * t + 2], wr[4 * t + 3]);
-                        *(uint4 *)(dst + 2 * PLANE + t * (BF_COLS * 16)) = make_uint4(wn[4 * t], wn[4 * t + 1], wn[4 * t + 2], wn[4 * t + 3]);
-                    }
-                fence_async_smem();
-                __syncwarp();
-                if (lane == 0) mbar_arrive(&a_full[buf]);
             }
+#pragma unroll
+            for (int t = 0; t < NCK; t++)
+                if (16 * (t + 1) > 7 * H) {  // trailing chunk(s) that the last element did not complete (zero padded)
+                    *(uint4 *)(dst + t * (BF_COLS * 16)) = make_uint4(wi[4 * t], wi[4 * t + 1], wi[4 * t + 2], wi[4 * t + 3]);
+                    *(uint4 *)(dst + PLANE + t * (BF_COLS * 16)) = make_uint4(wr[4 * t], wr[4 * t + 1], wr[4 * t + 2], wr[4 * t + 3]);
+                    *(uint4 *)(dst + 2 * PLANE + t * (BF_COLS * 16)) = make_uint4(wn[4 * t], wn[4 * t + 1], wn[4 * t + 2], wn[4 * t + 3]);
+                }
+            fence_async_smem();
+            __syncwarp();
+            if (lane == 0) mbar_arrive(&a_full[buf]);
         }
-    } else if (warp >= 8) {
+    } else if (warp >= 12) {
         // ------------------------------------------------ epilogue: thread = data column (TMEM lane), both parts
-        const int qd = (warp - 8) >> 2, row = (warp & 3) * 32 + lane;
+        const int qd = (warp - 12) >> 2, row = (warp & 3) * 32 + lane;
         const uint32_t lane_taddr = tmem + ((uint32_t)((warp & 3) * 32) << 16);
         uint32_t it = 0, u = 0;
         for (long long tile = blockIdx.x; tile < ntiles; tile += gridDim.x, it++) {
@@ -363,6 +380,10 @@ __global__ void __launch_bounds__(BF_THREADS, 1) stage_bf_kernel(StageGeom g, co
 #pragma unroll 1
                 for (int gg = 0; gg < 2; gg++, u++) {
                     if ((int)(u % 3) != qd) continue;
+                    const int kp = 2 * ch + gg;
+                    uint4 cc[2];
+                    cc[0] = __ldg(ct + (kp < H ? kp : 0));
+                    cc[1] = __ldg(ct + (kp < H ? kp + H : 0));
                     bf_wait(&pa_full[qd], (u / 3) & 1);
                     tc_fence_after();
                     uint32_t E[4][5];  // [part*2 + o]
@@ -376,12 +397,10 @@ __global__ void __launch_bounds__(BF_THREADS, 1) stage_bf_kernel(StageGeom g, co
                     tc_fence_before();
                     __syncwarp();
                     if (lane == 0) mbar_arrive(&pa_empty[qd]);
-                    const int kp = 2 * ch + gg;
                     if (kp >= H) continue;
 #pragma unroll
                     for (int o = 0; o < 2; o++) {
                         const int k = kp + o * H;
-                        const uint4 cc = __ldg(ct + k);
                         uint64_t y[2];
 #pragma unroll
                         for (int P = 0; P < 2; P++) {
@@ -391,7 +410,7 @@ __global__ void __launch_bounds__(BF_THREADS, 1) stage_bf_kernel(StageGeom g, co
                                 const uint32_t *e = E[P * 2 + o];
                                 uint32_t r[4], r2[4];
                                 crt_from_E(e[0], e[1], e[2], e[3], e[4], r);
-                                sub128(r2, r[0], r[1], r[2], r[3], cc.x, cc.y, cc.z, cc.w);
+                                sub128(r2, r[0], r[1], r[2], r[3], cc[o].x, cc[o].y, cc[o].z, cc[o].w);
                                 y[P] = pack_limbs(r2, gexp);
                             }
                         }
