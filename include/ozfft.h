@@ -68,6 +68,10 @@ size_t ozfft_debug_bf_tables(int K, int fusedN, int sign, void *h_B, void *h_C, 
  * exactly this to run Phase A on the stage accumulators without a SIMT pass.  Device pointers. */
 int ozfft_probe_chain(int n1, int kbytes, int n2, const void *dA, const void *dB1, const void *dB2, void *dD1, void *dD2,
                       void *stream);
+/* tcgen05.cp probe: A[128][kbytes] -> shared-memory operand chunks -> TMEM -> D[128][kbytes/4] 32-bit words; D must
+ * hold A's bytes unchanged (row r in lane r, 16 bytes = 4 columns).  The byte-fed kernel moves its data operand into
+ * TMEM this way once per tile.  kbytes multiple of 16, <= 1024.  Device pointers. */
+int ozfft_probe_cp(int kbytes, const void *dA, void *dD, void *stream);
 /* Device CRT probe (PAPER.md:316-329 direct CRT, 370-373 two-sided lift, Alg. 2 lines 9-13 at 408-413):
  * d_residues = n x 12 uint16 (any representative of each residue below 2^13), d_out = n x 4 uint32 = two's-complement
  * limbs of the centred result in [-M/2, M/2).  variant 1: the tensor-core form the stage kernels use (Phase-A MMA,

@@ -63,11 +63,14 @@ __device__ __forceinline__ uint64_t quantise_mag(uint64_t b, int Tmax) {
     return q;
 }
 
+// out-of-line copies of the rare paths: keeps the unrolled hot loops small enough for the instruction cache
+__device__ __noinline__ uint64_t quantise_mag_slow(uint64_t b, int Tmax) { return quantise_mag(b, Tmax); }
+
 // same value as quantise_mag; normal numbers (the usual case) take a short branch-free path:
 // q = mant >> sh, the dropped bits left-aligned give the guard bit and the sticky flag
 __device__ __forceinline__ uint64_t quantise_mag_fast(uint64_t b, int Tmax) {
     const int ef = (int)((b >> 52) & 0x7FF);
-    if (ef == 0) return quantise_mag(b, Tmax);  // zero or subnormal
+    if (ef == 0) return quantise_mag_slow(b, Tmax);  // zero or subnormal
     const uint64_t mant = (b & 0xFFFFFFFFFFFFFull) | (1ull << 52);
     const int sh = Tmax + 1023 - ef;  // >= 0 because Tmax is the column maximum
     if (sh == 0) return mant;
@@ -77,10 +80,7 @@ __device__ __forceinline__ uint64_t quantise_mag_fast(uint64_t b, int Tmax) {
         const uint32_t up = (dropped >> 31) & ((uint32_t)((dropped << 1) != 0) | qlo);
         return (((uint64_t)qhi << 32) | qlo) + up;  // qlo + 1 cannot carry: q < 2^53 means qhi:qlo + 1 fits
     }
-    if (sh > 54) return 0;            // below half a unit
-    const uint64_t q = mant >> sh, dropped = mant << (64 - sh);
-    const uint64_t up = (dropped >> 63) & ((uint64_t)((dropped << 1) != 0) | q);
-    return q + (up & 1);
+    return quantise_mag_slow(b, Tmax);  // more than 2^32 below the column maximum
 }
 
 // r in [0, 2^32) -> r mod m by Barrett with mu = floor(2^32/m): one multiply-high, one conditional subtract
@@ -152,6 +152,10 @@ __device__ __forceinline__ uint64_t pack_rne(i128 R, int g) {
     return sgn | q;
 }
 
+__device__ __noinline__ uint64_t pack_rne_slow(uint32_t r0, uint32_t r1, uint32_t r2, uint32_t r3, int g) {
+    return pack_rne((i128)(((u128)r3 << 96) | ((u128)r2 << 64) | ((u128)r1 << 32) | r0), g);
+}
+
 // Exact CRT of 12 canonical residues to the centred representative in [-M/2, M/2)
 // (PAPER.md:316-329 direct CRT with idempotents; 370-373 fractional lift and two-sided correction).
 // Plain multiword form used by the SIMT reference kernel: all sums are taken mod 2^128, which is exact
@@ -196,6 +200,17 @@ __device__ __forceinline__ void abs128(uint32_t *a, const uint32_t *x, uint32_t 
 // PAPER.md:370 with the fraction taken from E itself), R = E - zhat M, two-sided centring.
 // r[0..3]: two's-complement limbs of R in [-M/2, M/2).
 __device__ __forceinline__ void crt_from_E(uint32_t e0, uint32_t e1, uint32_t e2, uint32_t e3, uint32_t e4, uint32_t *r);
+
+// two-sided centring of a value already within one M of the centred range; out of line: in a
+// transform |R| <= 2^112.5 and the caller's top-limb test never sends it here (tests/test_gpu_crt.py does)
+__device__ __noinline__ uint4 centre_two_sided(uint32_t r0, uint32_t r1, uint32_t r2, uint32_t r3) {
+    const u128 M = ((u128)kc.M[3] << 96) | ((u128)kc.M[2] << 64) | ((u128)kc.M[1] << 32) | kc.M[0];
+    i128 R = (i128)(((u128)r3 << 96) | ((u128)r2 << 64) | ((u128)r1 << 32) | r0);
+    const i128 Mh = (i128)(M >> 1);
+    if (R >= Mh) R -= (i128)M;
+    if (R < -Mh) R += (i128)M;
+    return make_uint4((uint32_t)R, (uint32_t)((u128)R >> 32), (uint32_t)((u128)R >> 64), (uint32_t)((u128)R >> 96));
+}
 
 __device__ __forceinline__ void crt_limbs(const uint32_t *v, uint32_t *r) {
     uint64_t a0 = 0, a1 = 0, a2 = 0, a3 = 0;
@@ -248,12 +263,8 @@ __device__ __forceinline__ void crt_from_E(uint32_t e0, uint32_t e1, uint32_t e2
     sub128(r, e0, e1, e2, e3, (uint32_t)p0, (uint32_t)p1, (uint32_t)p2, (uint32_t)p3);
     // |R| can reach M/2 only if the top limb does; everything else skips the exact comparison
     if ((uint32_t)(r[3] + kc.Mh[3]) >= 2 * kc.Mh[3]) {
-        const u128 M = ((u128)kc.M[3] << 96) | ((u128)kc.M[2] << 64) | ((u128)kc.M[1] << 32) | kc.M[0];
-        i128 R = (i128)(((u128)r[3] << 96) | ((u128)r[2] << 64) | ((u128)r[1] << 32) | r[0]);
-        const i128 Mh = (i128)(M >> 1);
-        if (R >= Mh) R -= (i128)M;
-        if (R < -Mh) R += (i128)M;
-        r[0] = (uint32_t)R; r[1] = (uint32_t)((u128)R >> 32); r[2] = (uint32_t)((u128)R >> 64); r[3] = (uint32_t)((u128)R >> 96);
+        const uint4 c = centre_two_sided(r[0], r[1], r[2], r[3]);
+        r[0] = c.x; r[1] = c.y; r[2] = c.z; r[3] = c.w;
     }
 }
 
@@ -275,8 +286,7 @@ __device__ __forceinline__ uint64_t pack_limbs(const uint32_t *r, int g) {
     }
     const int X = 127 - s - g;
     if ((uint32_t)(X + 1022) > 2045u || s >= 128) {  // zero, subnormal or overflowing result: generic path
-        const i128 R = (i128)(((u128)r[3] << 96) | ((u128)r[2] << 64) | ((u128)r[1] << 32) | r[0]);
-        return pack_rne(R, g);
+        return pack_rne_slow(r[0], r[1], r[2], r[3], g);
     }
     const int bs = s & 31;
     const uint32_t m3 = __funnelshift_l(a2, a3, bs), m2 = __funnelshift_l(a1, a2, bs), m1 = __funnelshift_l(a0, a1, bs), m0 = a0 << bs;

@@ -205,6 +205,53 @@ __global__ void __launch_bounds__(128, 1) probe_crt_kernel(int variant, int n, c
 
 }  // namespace
 
+namespace {
+// A[128][kb] (row-major bytes) -> shared memory chunks [kb/16][128][16] -> tcgen05.cp into TMEM columns [0, kb/4)
+// -> tcgen05.ld -> D[128][kb/4] words; must reproduce A's bytes (little endian) word for word.
+__global__ void __launch_bounds__(128, 1) probe_cp_kernel(int kb, const uint8_t *A, uint32_t *D) {
+    extern __shared__ __align__(128) uint8_t smem[];
+    __shared__ uint64_t bar;
+    __shared__ uint32_t tmem_base_s;
+    const int tid = threadIdx.x, warp = tid >> 5;
+    for (int i = tid; i < 128 * (kb / 16); i += 128) {
+        int r = i % 128, c = i / 128;
+        *(uint4 *)(smem + (c * 128 + r) * 16) = *(const uint4 *)(A + (size_t)r * kb + c * 16);
+    }
+    if (warp == 0) tmem_alloc<512>(&tmem_base_s);
+    if (tid == 0) { mbar_init(&bar, 1); mbar_fence_init(); }
+    fence_async_smem();
+    tc_fence_before();
+    __syncthreads();
+    tc_fence_after();
+    const uint32_t tmem = tmem_base_s;
+    if (warp == 0) {
+        if (elect_one()) {
+            for (int c = 0; c < kb / 16; c++) tmem_cp_128x128b(tmem + 4 * c, make_sdesc(smem_u32(smem) + c * 2048, 2048, 128));
+            tc_commit(&bar);
+        }
+        __syncwarp();
+    }
+    mbar_wait(&bar, 0);
+    tc_fence_after();
+    for (int c = 0; c < kb / 4; c++) {
+        uint32_t v;
+        tmem_ld_x1(tmem + ((uint32_t)(warp * 32) << 16) + c, v);
+        tmem_ld_wait();
+        D[(size_t)tid * (kb / 4) + c] = v;
+    }
+    tc_fence_before();
+    __syncthreads();
+    if (warp == 0) tmem_dealloc<512>(tmem);
+}
+}  // namespace
+
+extern "C" int ozfft_probe_cp(int kbytes, const void *dA, void *dD, void *stream) {
+    if (kbytes < 16 || kbytes > 1024 || (kbytes % 16)) return OZFFT_EINVAL;
+    cudaFuncSetAttribute(probe_cp_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 128 * kbytes);
+    probe_cp_kernel<<<1, 128, 128 * kbytes, (cudaStream_t)stream>>>(kbytes, (const uint8_t *)dA, (uint32_t *)dD);
+    return cudaGetLastError() == cudaSuccess ? OZFFT_OK : OZFFT_ECUDA;
+}
+
 extern "C" int ozfft_probe_chain(int n1, int kbytes, int n2, const void *dA, const void *dB1, const void *dB2, void *dD1,
                                  void *dD2, void *stream) {
     if (n1 < 16 || n1 > 256 || (n1 % 16) || n2 < 16 || n2 > 256 || (n2 % 16) || kbytes < 32 || (kbytes % 32)) return OZFFT_EINVAL;

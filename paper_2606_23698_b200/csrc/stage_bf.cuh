@@ -130,20 +130,23 @@ inline void build_pa_bf(uint8_t *pa, const CrtConsts &C) {
 // warps 12-23 = epilogue (a7-a9, a12: deposits, lift, pack, store; three groups of four warps, one TMEM lane
 // quarter each).  All hand-offs are mbarriers; there is no block-wide barrier inside the tile loop.
 constexpr int BF_THREADS = 768;
-constexpr int BF_NSLOT = 4;         // matrix ring slots (one parity of one chunk each)
-constexpr int BF_DPA = 384;         // TMEM column of the Phase-A results: [slot g][part][o][16 slices]
+constexpr int BF_NSLOT = 12;        // matrix ring slots (one parity of one chunk each)
+// TMEM columns: [0,168) data operand (per parity 84: XI | XR | NXI, 4 columns per 16-byte chunk), [168,360) stage
+// accumulators of one chunk ([re rows: E 48 | O 48][im rows: E 48 | O 48]), [360,488) Phase-A results (2 slots x 64)
+constexpr int BF_TA = 0, BF_TD = 168, BF_DPA = 360;
 template <int K> __host__ __device__ constexpr size_t bf_smem_bytes() {
-    return 2 * (size_t)bf_aset_bytes(K) + (size_t)BF_NSLOT * bf_slot_bytes(K) + BF_PA_BYTES;
+    return (size_t)bf_aset_bytes(K) + (size_t)BF_NSLOT * bf_slot_bytes(K) + BF_PA_BYTES;
 }
 
-// bounded wait: a pipeline bug must not hang the GPU (traps after ~2^28 failed polls, i.e. several seconds)
+// bounded wait: a pipeline bug must not hang the GPU (traps after 2^22 failed polls of up to 1 ms each)
 __device__ __forceinline__ void bf_wait(uint64_t *bar, uint32_t parity) {
     const uint32_t a = smem_u32(bar);
     uint32_t done, spins = 0;
     do {
-        asm volatile("{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\tselp.u32 %0, 1, 0, p;\n\t}"
-                     : "=r"(done) : "r"(a), "r"(parity) : "memory");
-        if (!done && ++spins > (1u << 28)) __trap();
+        // the suspend-time hint lets the hardware park the warp instead of re-issuing the poll
+        asm volatile("{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2, %3;\n\tselp.u32 %0, 1, 0, p;\n\t}"
+                     : "=r"(done) : "r"(a), "r"(parity), "r"(1000000u) : "memory");
+        if (!done && ++spins > (1u << 22)) __trap();
     } while (!done);
 }
 
@@ -167,10 +170,10 @@ __global__ void __launch_bounds__(BF_THREADS, 1) stage_bf_kernel(StageGeom g, co
     constexpr int SB = bf_slot_bytes(K), PLANE = bf_plane_bytes(K), ASET = bf_aset_bytes(K), PARB = NCK * BF_COLS * 16;
     constexpr int NW = PB / 4;
     extern __shared__ __align__(128) uint8_t smem[];
-    __shared__ __align__(8) uint64_t a_full[2], a_empty[2], b_full[BF_NSLOT], b_empty[BF_NSLOT], pa_full[3], pa_empty[3], st_done[2], d_free[2];
+    __shared__ __align__(8) uint64_t a_full[1], a_empty[1], e_start[1], b_full[BF_NSLOT], b_empty[BF_NSLOT], pa_full[3], pa_empty[3];
     __shared__ uint32_t s_tmem;
     __shared__ int s_T[2][BF_COLS], s_flag[2][BF_COLS];
-    uint8_t *sA = smem, *sB = smem + 2 * ASET, *sPA = sB + BF_NSLOT * SB;
+    uint8_t *sA = smem, *sB = smem + ASET, *sPA = sB + BF_NSLOT * SB;
 
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     const int lg_nbt = 32 - __clz(((g.nb + 3) >> 2) - 1), lg_ns = 31 - __clz(g.ns);
@@ -180,7 +183,7 @@ __global__ void __launch_bounds__(BF_THREADS, 1) stage_bf_kernel(StageGeom g, co
     if (tid == 0) {
         // pa_full / pa_empty are per epilogue group (a waiter must see every phase of its barrier in turn:
         // try_wait on parity p passes at once while the barrier is still in the phase before p)
-        for (int i = 0; i < 2; i++) { mbar_init(&a_full[i], 8); mbar_init(&a_empty[i], 13); mbar_init(&st_done[i], 1); mbar_init(&d_free[i], 1); }
+        mbar_init(&a_full[0], 8); mbar_init(&a_empty[0], 1); mbar_init(&e_start[0], 12);
         for (int i = 0; i < 3; i++) { mbar_init(&pa_full[i], 1); mbar_init(&pa_empty[i], 4); }
         for (int i = 0; i < BF_NSLOT; i++) { mbar_init(&b_full[i], 1); mbar_init(&b_empty[i], 1); }
         mbar_fence_init();
@@ -209,19 +212,31 @@ __global__ void __launch_bounds__(BF_THREADS, 1) stage_bf_kernel(StageGeom g, co
             }
         }
     } else if (warp == 1) {
-        // ------------------------------------------------ stage MMA issuer: a4 (with a3 and a5 folded into the operands)
-        // every descriptor is one base plus a compile-time constant (address in 16-byte units in bits 0-13, the
-        // leading-dimension byte offset in bits 16-29)
-        const uint32_t idesc_st = make_idesc(CFMT_S32, I8_U8, I8_U8, 128, BF_N);
-        const uint64_t bdesc0 = make_sdesc(smem_u32(sB), BF_N * 16, 128);
+        // ------------------------------------------------ tensor-core issuer (one elected lane; program order = execution order)
+        // per tile: tcgen05.cp of the data operand shared memory -> TMEM (then the shared copy is free for the next
+        // tile); per chunk: a4 stage MMAs with A from TMEM (a3 and a5 folded into the operands), then a6 Phase A with
+        // A = the stage accumulators.  Every descriptor is one base plus a compile-time constant.
+        const uint32_t idesc_st = make_idesc(CFMT_S32, I8_U8, I8_U8, 128, BF_N), idesc_pa = make_idesc(CFMT_S32, I8_U8, I8_U8, 128, 32);
+        const uint64_t bdesc0 = make_sdesc(smem_u32(sB), BF_N * 16, 128), pdesc0 = make_sdesc(smem_u32(sPA), 32 * 16, 128);
+        const uint64_t adesc0 = make_sdesc(smem_u32(sA), BF_COLS * 16, 128);
+        constexpr int ACOLS = 3 * NCK * 4;  // TMEM columns of one parity of the data operand
         uint32_t m = 0, n = 0, it = 0;
         for (long long tile = blockIdx.x; tile < ntiles; tile += gridDim.x, it++) {
-            const uint32_t buf = it & 1;
-            bf_wait(&a_full[buf], (it >> 1) & 1);
-            const uint64_t adesc0 = make_sdesc(smem_u32(sA) + buf * ASET, BF_COLS * 16, 128);
+            bf_wait(&a_full[0], it & 1);
+            tc_fence_after();
+            if (elect_one()) {
+#pragma unroll
+                for (int par = 0; par < 2; par++)
+#pragma unroll
+                    for (int pl = 0; pl < 3; pl++)
+#pragma unroll
+                        for (int t = 0; t < NCK; t++)
+                            tmem_cp_128x128b(tmem + BF_TA + par * ACOLS + (pl * NCK + t) * 4,
+                                             adesc0 + (uint64_t)((pl * PLANE + par * PARB + t * (BF_COLS * 16)) >> 4));
+                tc_commit(&a_empty[0]);
+            }
+            __syncwarp();
             for (int ch = 0; ch < NCH; ch++, n++) {
-                const uint32_t q = n & 1;
-                if (n >= 2) bf_wait(&d_free[q], ((n >> 1) - 1) & 1);  // Phase A of chunk n-2 has read this accumulator buffer
 #pragma unroll
                 for (int par = 0; par < 2; par++, m++) {
                     const uint32_t slot = m % BF_NSLOT;
@@ -230,34 +245,15 @@ __global__ void __launch_bounds__(BF_THREADS, 1) stage_bf_kernel(StageGeom g, co
                     if (elect_one()) {
                         const uint64_t bd = bdesc0 + (uint64_t)((slot * SB) >> 4);
 #pragma unroll
-                        for (int P = 0; P < 2; P++)  // P = 0: re rows [XR ; NXI], P = 1: im rows [XI ; XR]
+                        for (int P = 0; P < 2; P++)  // P = 0: re rows [XR ; NXI] (planes 1, 2), P = 1: im rows [XI ; XR] (planes 0, 1)
 #pragma unroll
-                            for (int s = 0; s < NCK; s++) {  // K step s = logical chunks 2s, 2s+1 of [block 0 | block 1]
-                                const int L0 = 2 * s, L1 = 2 * s + 1;
-                                const int o0 = (1 - P) * PLANE + par * PARB + (L0 / NCK) * PLANE + (L0 % NCK) * (BF_COLS * 16);
-                                const int o1 = (1 - P) * PLANE + par * PARB + (L1 / NCK) * PLANE + (L1 % NCK) * (BF_COLS * 16);
-                                const uint64_t acon = (uint64_t)(o0 >> 4) + ((uint64_t)((o1 - o0 - BF_COLS * 16) >> 4) << 16);
-                                mma_i8_ss(tmem + q * 192 + P * 96 + par * 48, adesc0 + acon, bd + (uint64_t)((s * 2 * BF_N * 16) >> 4), idesc_st, s > 0);
-                            }
+                            for (int s = 0; s < NCK; s++)  // K step s = chunks 2s, 2s+1 of the two adjacent planes
+                                mma_i8_ts(tmem + BF_TD + P * 96 + par * 48, tmem + BF_TA + par * ACOLS + ((1 - P) * NCK + 2 * s) * 4,
+                                          bd + (uint64_t)((s * 2 * BF_N * 16) >> 4), idesc_st, s > 0);
                         tc_commit(&b_empty[slot]);
-                        if (par == 1) {
-                            tc_commit(&st_done[q]);
-                            if (ch == NCH - 1) tc_commit(&a_empty[buf]);
-                        }
                     }
                     __syncwarp();
                 }
-            }
-        }
-    } else if (warp == 2) {
-        // ------------------------------------------------ Phase-A MMA issuer: a6, A operand = the stage accumulators in TMEM
-        const uint32_t idesc_pa = make_idesc(CFMT_S32, I8_U8, I8_U8, 128, 32);
-        const uint64_t pdesc0 = make_sdesc(smem_u32(sPA), 32 * 16, 128);
-        uint32_t n = 0;
-        for (long long tile = blockIdx.x; tile < ntiles; tile += gridDim.x)
-            for (int ch = 0; ch < NCH; ch++, n++) {
-                const uint32_t q = n & 1;
-                bf_wait(&st_done[q], (n >> 1) & 1);
 #pragma unroll
                 for (int gg = 0; gg < 2; gg++) {
                     const uint32_t u = 2 * n + gg;  // unit index; its D_PA slot gg was last used by unit u - 2
@@ -268,14 +264,14 @@ __global__ void __launch_bounds__(BF_THREADS, 1) stage_bf_kernel(StageGeom g, co
                         for (int P = 0; P < 2; P++)
 #pragma unroll
                             for (int s = 0; s < 6; s++)
-                                mma_i8_ts(tmem + BF_DPA + gg * 64 + P * 32, tmem + q * 192 + P * 96 + (s >= 3 ? 48 : 0) + gg * 24 + (s % 3) * 8,
+                                mma_i8_ts(tmem + BF_DPA + gg * 64 + P * 32, tmem + BF_TD + P * 96 + (s >= 3 ? 48 : 0) + gg * 24 + (s % 3) * 8,
                                           pdesc0 + (uint64_t)((s * 2 * 32 * 16) >> 4), idesc_pa, s > 0);
                         tc_commit(&pa_full[u % 3]);
-                        if (gg == 1) tc_commit(&d_free[q]);
                     }
                     __syncwarp();
                 }
             }
+        }
     } else if (warp >= 4 && warp < 12) {
         // ------------------------------------------------ deconstruction: thread = (column, parity of j)
         const int dw = warp - 4, par = lane >> 4, c = dw * 16 + (lane & 15);
@@ -312,14 +308,14 @@ __global__ void __launch_bounds__(BF_THREADS, 1) stage_bf_kernel(StageGeom g, co
                 tm = max(tm, __shfl_xor_sync(0xFFFFFFFFu, tm, 16));
                 if (ef == 0 && tm > -100000) { flag = 1; Tmax = tm; }
             }
-            // the previous user of this operand buffer (the stage MMAs of tile it-2) must be done before the writes
-            if (it >= 2) bf_wait(&a_empty[buf], ((it >> 1) - 1) & 1);
+            // the previous tile's operand must have been copied to TMEM before the shared copy is overwritten
+            if (it >= 1) bf_wait(&a_empty[0], (it - 1) & 1);
             if (par == 0) { s_T[buf][c] = Tmax; s_flag[buf][c] = flag; }
             // a3: quantise, offset by 2^53, split into bytes; planes XI (0), XR (1), NXI (2)
             uint32_t wr[NW + 2], wi[NW + 2], wn[NW + 2];
 #pragma unroll
             for (int t = 0; t < NW + 2; t++) wr[t] = wi[t] = wn[t] = 0;
-            uint8_t *dst = sA + buf * ASET + par * PARB + c * 16;
+            uint8_t *dst = sA + par * PARB + c * 16;
 #pragma unroll
             for (int e0 = 0; e0 < H; e0 += BS) {
                 uint4 vv[BS];
@@ -353,9 +349,12 @@ __global__ void __launch_bounds__(BF_THREADS, 1) stage_bf_kernel(StageGeom g, co
                     *(uint4 *)(dst + PLANE + t * (BF_COLS * 16)) = make_uint4(wr[4 * t], wr[4 * t + 1], wr[4 * t + 2], wr[4 * t + 3]);
                     *(uint4 *)(dst + 2 * PLANE + t * (BF_COLS * 16)) = make_uint4(wn[4 * t], wn[4 * t + 1], wn[4 * t + 2], wn[4 * t + 3]);
                 }
+            // every epilogue warp must have observed the a_full phase of tile it-1 (and read its exponents) before
+            // this tile's phase may complete: a waiter that falls two phases behind would wait forever
+            if (it >= 1) bf_wait(&e_start[0], (it - 1) & 1);
             fence_async_smem();
             __syncwarp();
-            if (lane == 0) mbar_arrive(&a_full[buf]);
+            if (lane == 0) mbar_arrive(&a_full[0]);
         }
     } else if (warp >= 12) {
         // ------------------------------------------------ epilogue: thread = data column (TMEM lane), both parts
@@ -370,10 +369,10 @@ __global__ void __launch_bounds__(BF_THREADS, 1) stage_bf_kernel(StageGeom g, co
             const bool valid = blk < g.nb;
             uint4 *dstp = out + ((long long)blk * g.ob + (long long)ts * g.os + (long long)to * g.oo + (long long)(row & 31) * g.lane);
             const uint4 *ct = ctab + (size_t)(g.matsel ? ts : 0) * K;
-            bf_wait(&a_full[buf], (it >> 1) & 1);
-            const int Tmax = s_T[buf][row], flag = s_flag[buf][row];
+            bf_wait(&a_full[0], it & 1);  // the column exponents of this tile are published (s_T is double buffered: the
+            const int Tmax = s_T[buf][row], flag = s_flag[buf][row];  // deconstruction runs at most one tile ahead)
             __syncwarp();
-            if (lane == 0) mbar_arrive(&a_empty[buf]);
+            if (lane == 0) mbar_arrive(&e_start[0]);
             const int gexp = 53 + 52 - Tmax;
 #pragma unroll 1
             for (int ch = 0; ch < NCH; ch++)

@@ -107,6 +107,13 @@ __device__ __forceinline__ void mma_i8_ts(uint32_t tmem_d, uint32_t tmem_a, uint
                  : "memory");
 }
 
+// shared memory -> TMEM copy of one 16-byte K chunk of a 128-row operand (canonical no-swizzle layout: 8-row groups
+// of 128 contiguous bytes, SBO apart): row r lands in lane r, the 16 bytes in four consecutive 32-bit columns.
+// Ordered with the MMAs issued by the same thread.
+__device__ __forceinline__ void tmem_cp_128x128b(uint32_t taddr, uint64_t sdesc) {
+    asm volatile("tcgen05.cp.cta_group::1.128x128b [%0], %1;" ::"r"(taddr), "l"(sdesc) : "memory");
+}
+
 // ---- TMEM <-> registers: 32 lanes x 32 bit, N consecutive columns; warp w touches lanes 32*(w%4).. ----
 __device__ __forceinline__ void tmem_ld_wait() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
 __device__ __forceinline__ void tmem_st_wait() { asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory"); }

@@ -12,7 +12,7 @@ _lib = None
 
 SYMBOLS = ["ozfft_plan_create", "ozfft_plan_create_1d", "ozfft_exec", "ozfft_exec_host", "ozfft_plan_destroy",
            "ozfft_last_error", "ozfft_twiddle_checksum", "ozfft_plan_num_launches", "ozfft_plan_device_bytes",
-           "ozfft_exec_axis", "ozfft_probe_mma", "ozfft_probe_chain", "ozfft_probe_crt", "ozfft_debug_bf_tables"]
+           "ozfft_exec_axis", "ozfft_probe_mma", "ozfft_probe_chain", "ozfft_probe_crt", "ozfft_debug_bf_tables", "ozfft_probe_cp"]
 
 
 def lib():
@@ -39,6 +39,7 @@ def lib():
         L.ozfft_probe_mma.argtypes = [C.c_int, C.c_int, C.c_int, vp, vp, vp, vp]
         L.ozfft_probe_chain.argtypes = [C.c_int, C.c_int, C.c_int, vp, vp, vp, vp, vp, vp]
         L.ozfft_probe_crt.argtypes = [C.c_int, vp, vp, C.c_int, vp]
+        L.ozfft_probe_cp.argtypes = [C.c_int, vp, vp, vp]
         L.ozfft_debug_bf_tables.restype = C.c_size_t
         L.ozfft_debug_bf_tables.argtypes = [C.c_int, C.c_int, C.c_int, vp, vp, vp]
         _lib = L
@@ -172,3 +173,13 @@ def debug_bf_tables(K, fusedN, sign):
     PA = np.zeros(6144, dtype=np.uint8)
     lib().ozfft_debug_bf_tables(K, fusedN, sign, B.ctypes.data, Cc.ctypes.data, PA.ctypes.data)
     return B, Cc, PA
+
+
+def probe_cp(A):
+    """A: uint8 CUDA [128, kb] -> uint8 CUDA [128, kb] read back from TMEM after a tcgen05.cp of every 16-byte chunk."""
+    import torch
+    kb = A.shape[1]
+    D = torch.zeros((128, kb // 4), dtype=torch.int32, device=A.device)
+    _check(lib().ozfft_probe_cp(kb, A.data_ptr(), D.data_ptr(), _stream(None)), "ozfft_probe_cp")
+    torch.cuda.synchronize()
+    return D.view(torch.uint8).reshape(128, kb)

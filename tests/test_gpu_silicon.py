@@ -90,3 +90,13 @@ def test_i8_mma_reads_s32_accumulators_from_tmem_as_bytes(n1, kb, n2):
     assert np.array_equal(D1, want1)
     by = np.ascontiguousarray(want1.astype(np.uint32)).view(np.uint8).reshape(128, 4 * n1)  # little-endian bytes
     assert np.array_equal(D2, by.astype(np.int64) @ B2.astype(np.int64).T)
+
+
+@pytest.mark.parametrize("kb", [16, 112, 672])
+def test_tcgen05_cp_moves_operand_chunks_into_tmem(kb):
+    """shared memory -> TMEM copy (tcgen05.cp 128x128b) of the byte-fed kernel's data operand: bytes unchanged"""
+    import torch
+    from paper_2606_23698_b200 import ozfft
+    A = np.random.default_rng(kb).integers(0, 256, (128, kb), dtype=np.uint8)
+    got = ozfft.probe_cp(torch.from_numpy(A).cuda()).cpu().numpy()
+    assert np.array_equal(got, A)
