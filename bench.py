@@ -97,11 +97,30 @@ def max_over_ranks(values, device="cpu"):
     return [float(v) for v in t]
 
 
-# DRAM bytes of one stage launch at 1024^3 from the committed ncu capture (profiles/r1_final.md):
-# dram__bytes_read.sum + dram__bytes_write.sum = 17.19 + 17.14 GB against 34.36 GB algorithmic
-NCU_TRAFFIC_PER_LAUNCH = {1024: 3.4334e10}
-# smsp__inst_executed.sum x 32 / n_out of the same capture (predicated-off lanes included)
-NCU_THREAD_INST_PER_OUT = 372.0
+def kernel_source_hash():
+    """sha256 over the kernel sources (csrc/*, include/*): ties a stored ncu figure to the code it was measured on"""
+    import glob
+    import hashlib
+    h = hashlib.sha256()
+    for f in sorted(glob.glob(os.path.join(ROOT, "paper_2606_23698_b200", "csrc", "*")) + glob.glob(os.path.join(ROOT, "include", "*.h"))):
+        h.update(os.path.basename(f).encode())
+        h.update(open(f, "rb").read())
+    return h.hexdigest()[:16]
+
+
+def ncu_constants(size, variant):
+    """ncu-derived figures of the dominant kernel (DRAM traffic per launch, thread instructions per output-equivalent)
+    from profiles/ncu_constants.json, which records the ncu command and the source hash they were measured on.
+    Returns (entry or None, note): None when no entry matches this size / variant / source hash (never a stale number)."""
+    try:
+        db = json.load(open(os.path.join(ROOT, "profiles", "ncu_constants.json")))
+    except Exception:
+        return None, "profiles/ncu_constants.json missing"
+    if db.get("source_hash") != kernel_source_hash():
+        return None, f"stale: profiles/ncu_constants.json was captured on source hash {db.get('source_hash')}, the tree is {kernel_source_hash()}"
+    e = db.get("entries", {}).get(f"{variant}:{size}")
+    return (e, db.get("command", "")) if e else (None, f"no ncu capture for variant {variant} at size {size}")
+
 
 
 def cpu_oracle_sample(size, pencils):
@@ -115,6 +134,11 @@ def cpu_oracle_sample(size, pencils):
     t = time.perf_counter()
     oracle.fft1d(x, -1, route=0)
     return time.perf_counter() - t, oracle.num_threads()
+
+
+def workload_name(size):
+    """the same string in both arms (the driver compares them)"""
+    return f"forward 3-D FFT {size}^3 complex128, uniform[-1,1), seed {SEED}" + (" (BASELINE.json configs[4])" if size == 1024 else "")
 
 
 def run_reference(args):
@@ -135,10 +159,11 @@ def run_reference(args):
     t_full = t_step * total_pencils / pencils  # extrapolated time of one whole transform
     val = flops(n_tot) / t_full / 1e9
     sample = f"{pencils} of {total_pencils} length-{size} pencils per step ({pencils / total_pencils:.4%} of one transform), extrapolated"
+    workload = workload_name(size)
     line = {"impl": "reference", "metric": "emulated_fp64_fft3d_gflops_5NlogN", "value": val, "unit": "GFLOP/s",
             "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup, "ms_per_step": t_full * 1e3,
             "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "int128", "data": "synthetic",
-            "config": {"workload": f"forward 3-D FFT {size}^3 complex128, uniform[-1,1), seed {SEED}"},
+            "config": {"workload": workload},
             "cpu_baseline": {"value": val, "unit": "GFLOP/s", "cores": threads, "kind": "oracle", "sample": sample},
             "e2e": {"value": val, "unit": "GFLOP/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
             "gpu_launches": 0}
@@ -154,6 +179,18 @@ def run_ours(args):
     world = int(os.environ.get("WORLD_SIZE", "1"))
     rank = int(os.environ.get("RANK", "0"))
     local = int(os.environ.get("LOCAL_RANK", "0"))
+    if world != args.gpus:
+        raise SystemExit(f"bench.py: --gpus {args.gpus} but WORLD_SIZE={world}: launch with torchrun --nproc-per-node {args.gpus} "
+                         f"(or run `python bench.py --gpus {args.gpus}` without WORLD_SIZE set: it spawns the ranks itself)")
+    if args.dry_run:  # CPU rehearsal of the launch plumbing only (tests/test_multirank_cpu.py): no transform is run
+        if world > 1:
+            dist.init_process_group("gloo")
+        worst = max_over_ranks([float(rank)])
+        if rank == 0:
+            print(json.dumps({"dry_run": True, "n_gpus": world, "max_rank_seen": worst[0]}))
+        if world > 1:
+            dist.destroy_process_group()
+        return
     if not torch.cuda.is_available():
         raise SystemExit("bench.py needs a B200: there is no CPU fallback")
     torch.cuda.set_device(local)
@@ -269,35 +306,46 @@ def run_ours(args):
 
     if rank == 0:
         peak, peak_src = peaks()
-        alg_bytes_launch = 32.0 * n_tot  # 16 B read + 16 B write per element per stage launch
+        variant = os.environ.get("OZFFT_VARIANT", "bf")
+        # algorithmic bytes = 32 B per element per AXIS PASS (16 read + 16 written) =
+        # 96 N_tot per transform; a transform is `launches` stage launches of one kernel (two per axis when n > 32), so
+        # one launch accounts for 96 N_tot / launches algorithmic bytes.  The measured DRAM traffic of a launch is
+        # 32 N_tot (the intermediate array Y' crosses HBM: beta = 2, reported beside the fraction).
+        alg_bytes_launch = 96.0 * n_tot / launches
         launch_ms = ms_step / launches
         achieved = alg_bytes_launch / (launch_ms * 1e-3) / 1e9
+        ncu, ncu_note = ncu_constants(size, variant)
+        traffic = ncu["dram_bytes_per_launch"] if ncu else None
+        tinst = ncu["thread_inst_per_output_eq"] if ncu else None
         line = {
             "metric": "emulated_fp64_fft3d_gflops_5NlogN", "value": world * flops(n_tot) / (ms_step_max * 1e-3) / 1e9,
             "unit": "GFLOP/s", "n_gpus": world, "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms_step_max,
             "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "int32", "data": "synthetic",
-            "config": {"workload": f"forward 3-D FFT {size}^3 complex128, uniform[-1,1), seed {SEED} (BASELINE.json configs[4])",
+            "config": {"workload": workload_name(size),
                        "parallelism": "replicas only" if world > 1 else "single GPU", "l2": "inputs_exceed_l2" if nbytes > (126 << 20) else "l2_resident",
-                       "variant": os.environ.get("OZFFT_VARIANT", "bf"), "stage_launches_per_transform": launches},
+                       "variant": variant, "stage_launches_per_transform": launches},
             "ms_per_transform": ms_step_max, "ms_per_transform_min": min(ms), "inverse_ms": inv_ms,
             "roundtrip_rel_err": roundtrip, "host_and_device_paths_bit_identical": same,
             "hbm_roof": {"alg_bytes": 96.0 * n_tot if launches == 6 else alg_bytes_launch * launches / 2,
                          "roof_ms_at_measured_peak": 96.0 * n_tot / (peak * 1e9) * 1e3, "frac_of_roof": (96.0 * n_tot / (peak * 1e9) * 1e3) / ms_step},
             "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                         "traffic": NCU_TRAFFIC_PER_LAUNCH.get(size), "kernel": "stage kernel (all launches of a transform are this kernel)",
-                         "peak_source": peak_src, "alg_bytes_per_launch": alg_bytes_launch, "launch_ms": launch_ms},
+                         "traffic": traffic, "beta": (traffic / alg_bytes_launch if traffic else None),
+                         "kernel": {"bf": "stage_bf_kernel", "tc": "stage_tc_kernel", "simt": "stage_simt_kernel"}.get(variant, variant) + " (every launch of a transform is this kernel)",
+                         "peak_source": peak_src, "alg_bytes_per_launch": alg_bytes_launch, "launch_ms": launch_ms,
+                         "ncu": ncu_note},
             "clocks": clocks,
             "e2e": ({"value": world * flops(n_tot) / (e2e_ms_max * 1e-3) / 1e9, "unit": "GFLOP/s", "ms": e2e_ms_max,
                      "h2d_bytes_per_step": nbytes, "d2h_bytes_per_step": nbytes, "steps": e2e_steps} if host_ok else
                     {"value": None, "unit": "GFLOP/s", "h2d_bytes_per_step": nbytes, "d2h_bytes_per_step": nbytes,
                      "skipped": "not enough host memory on this node for N x 2 x 16 GiB of pinned buffers"}),
             "gpu_launches": launches * args.steps,
-            # what actually binds: SIMT integer issue.  achieved = n_out x the ncu-measured thread
-            # instructions per output-equivalent (profiles/r1_final.md) / step time; peak = 148 SM x 128 lanes x 1.965 GHz
-            "roofline_alu": {"bound": "alu", "achieved": 2 * launches * n_tot * NCU_THREAD_INST_PER_OUT / (ms_step * 1e-3) / 1e12,
-                             "peak": 148 * 128 * 1.965e9 / 1e12, "unit": "T thread-inst/s",
-                             "frac": 2 * launches * n_tot * NCU_THREAD_INST_PER_OUT / (ms_step * 1e-3) / (148 * 128 * 1.965e9),
-                             "n_out": 2 * launches * n_tot, "thread_inst_per_output_eq": NCU_THREAD_INST_PER_OUT},
+            # the SIMT side (PAPER.md:452 names integer issue as the wall): achieved = n_out x the ncu-measured thread
+            # instructions per output-equivalent / step time; peak = 148 SM x 128 lanes x 1.965 GHz.
+            # null when no ncu capture matches the current kernel sources.
+            "roofline_alu": ({"bound": "alu", "achieved": 2 * launches * n_tot * tinst / (ms_step * 1e-3) / 1e12,
+                              "peak": 148 * 128 * 1.965e9 / 1e12, "unit": "T thread-inst/s",
+                              "frac": 2 * launches * n_tot * tinst / (ms_step * 1e-3) / (148 * 128 * 1.965e9),
+                              "n_out": 2 * launches * n_tot, "thread_inst_per_output_eq": tinst} if tinst else None),
             "context": {"cufft_z2z_ms": cufft_ms, "paper_projection_ms_B300": [63, 87], "paper_projection_ms_B200": [70, 96],
                         "paper_hbm_roof_ms": 12.9},
         }
@@ -313,6 +361,61 @@ def run_ours(args):
         dist.destroy_process_group()
 
 
+def run_configs(args):
+    """--configs: ms per transform for all five BASELINE.json workloads (bench.py's contract line times only the headline
+    one): CUDA events on the current stream, median of --steps after --warmup; 5 N log2 N GFLOP/s; fraction of the HBM roof
+    (32 B per element per axis pass over the measured copy bandwidth); cuFFT Z2Z fp64 on the same tensor for context.
+    One JSON line per config, variant from OZFFT_VARIANT (default: the byte-fed kernel)."""
+    import torch
+    from paper_2606_23698_b200 import inputs, ozfft
+    hbm, _ = peaks()
+
+    def timed(fn):
+        for _ in range(max(3, args.warmup)):
+            fn()
+        torch.cuda.synchronize()
+        ts = []
+        for _ in range(args.steps):
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            fn()
+            e1.record()
+            torch.cuda.synchronize()
+            ts.append(e0.elapsed_time(e1))
+        ts.sort()
+        return ts[len(ts) // 2], ts[0]
+
+    for name, (kind, shape, dist_name, seed) in inputs.CONFIGS.items():
+        h = torch.empty(shape, dtype=torch.complex128)
+        if dist_name == "uniform":
+            inputs.uniform_pm1(shape, seed, out=h.numpy())
+        else:
+            h.copy_(torch.from_numpy(inputs.make(dist_name, shape, seed)))
+        x = h.cuda()
+        y = torch.empty_like(x)
+        if kind == "3d":
+            plan = ozfft.Plan(*shape)
+            flop, passes = 5.0 * x.numel() * math.log2(x.numel()), 3
+            cufft = lambda: torch.fft.fftn(x)
+        else:
+            plan = ozfft.Plan.batched_1d(shape[1], shape[0])
+            flop, passes = 5.0 * x.numel() * math.log2(shape[1]), 1
+            cufft = lambda: torch.fft.fft(x, dim=1)
+        med, best = timed(lambda: plan.exec(x, y))
+        try:
+            cmed, _ = timed(cufft)
+        except Exception:
+            cmed = None
+        roof_ms = 32.0 * x.numel() * passes / (hbm * 1e9) * 1e3
+        print(json.dumps({"config": name, "variant": os.environ.get("OZFFT_VARIANT", "bf"), "shape": list(shape), "input": dist_name,
+                          "seed": seed, "launches": plan.num_launches, "ms_median": med, "ms_best": best,
+                          "gflops_5NlogN": flop / (med * 1e-3) / 1e9, "hbm_roof_ms": roof_ms, "frac_of_hbm_roof": roof_ms / med,
+                          "cufft_z2z_ms": cmed}), flush=True)
+        plan.destroy()
+        del x, y, h
+        torch.cuda.empty_cache()
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -321,8 +424,21 @@ def main():
     ap.add_argument("--size", type=int, default=1024)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg (profiling runs)")
+    ap.add_argument("--configs", action="store_true", help="time all five BASELINE.json configs (one JSON line each) instead of the contract line")
+    ap.add_argument("--dry-run", action="store_true", help="launch plumbing only (gloo, no GPU work): used by the CPU tests")
     args = ap.parse_args()
-    if args.impl == "reference":
+    if args.gpus > 1 and "WORLD_SIZE" not in os.environ:
+        # `python bench.py --gpus N`: spawn the N ranks ourselves (one process per GPU, the driver's own launch line)
+        import socket
+        with socket.socket() as sk:
+            sk.bind(("127.0.0.1", 0))
+            port = sk.getsockname()[1]
+        cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={args.gpus}", "--master-addr", "127.0.0.1",
+               "--master-port", str(port), os.path.abspath(__file__)] + sys.argv[1:]
+        raise SystemExit(subprocess.call(cmd))
+    if args.configs:
+        run_configs(args)
+    elif args.impl == "reference":
         run_reference(args)
     else:
         run_ours(args)

@@ -7,13 +7,18 @@
  * rounded pack per stage output (Alg. 2).
  *
  * Conventions (readings S1..S8): sign = -1 forward (w_N = exp(-2 pi i/N)), +1 inverse, never
- * normalised.  Sizes are powers of two, 2 <= n <= 1024 per axis.  Arrays are row-major, z fastest:
+ * normalised.  Sizes are powers of two, 2 <= n <= 1024 per axis (every such shape is accepted; a batched 1-D plan takes
+ * any batch >= 1 with n * batch <= 2^30).  Arrays are row-major, z fastest:
  * element (x,y,z) at index (x*ny + y)*nz + z; one element = {re, im} as two IEEE-754 binary64 (16 bytes).
  * `in` and `out` are DEVICE pointers, 16-byte aligned, must not overlap; `in` is read only, `out` is fully
  * overwritten.  Inputs must be finite; a column holding a non-finite value produces NaN in the outputs of
  * that 1-D transform stage.  All plan memory (tables, workspace) is owned by the plan; the caller owns in/out.
  * ozfft_exec is asynchronous and ordered on `stream` (a cudaStream_t passed as void*); it never synchronises.
- * A plan must not execute concurrently on two streams (it owns workspace).  No CPU fallback exists.
+ * A plan must not execute concurrently on two streams (it owns workspace); different plans may be created and
+ * executed from different host threads.  A destroyed or unknown handle is refused with OZFFT_EINVAL (the library
+ * keeps a registry of live plans; it never dereferences a stale pointer).  Kernel selection: environment variable
+ * OZFFT_VARIANT = bf (default: byte-fed tensor-core kernel), tc (residue-digit tensor-core kernel), simt, read at
+ * plan creation.  No CPU fallback exists.
  */
 #ifndef OZFFT_H
 #define OZFFT_H

@@ -25,8 +25,6 @@ def build(force=False, verbose=False):
            "-o", SO] + sources() + ["-lcudart"]
     if verbose:
         cmd.insert(1, "-Xptxas=-v")
-    if os.environ.get("OZFFT_NVCC_FLAGS"):  # experiments only (e.g. -DTC_Q32=8)
-        cmd[1:1] = os.environ["OZFFT_NVCC_FLAGS"].split()
     subprocess.check_call(cmd)
     return SO
 

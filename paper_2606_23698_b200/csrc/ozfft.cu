@@ -6,6 +6,8 @@
 #include <cstdlib>
 #include <cstring>
 #include <map>
+#include <mutex>
+#include <set>
 #include <string>
 #include <vector>
 
@@ -31,10 +33,14 @@ bool cuda_ok(cudaError_t e, const char *what) {
 
 const Twiddles &twiddles() {
     static Twiddles T;
-    static bool init = false;
-    if (!init) { build_twiddles(T); init = true; }
+    static std::once_flag once;
+    std::call_once(once, [] { build_twiddles(T); });
     return T;
 }
+
+// live plans: a destroyed (or never created) handle is recognised without touching freed memory
+std::mutex g_plans_mu;
+std::set<const void *> g_plans;
 
 struct StageLaunch {
     StageGeom g;
@@ -53,6 +59,7 @@ struct ozfft_plan_s {
     long long count;
     int variant;  // 0 simt, 1 tensor-core (residue digits), 2 byte-fed tensor-core (default)
     int sms;      // SM count of the plan's device
+    int tc_per_sm[3];  // resident CTAs per SM of the residue-digit kernel instantiations (per device)
     const void *pa_bf;  // Phase-A constant matrix of the byte-fed kernel
     std::vector<StageLaunch> stages;
     std::vector<void *> dev_allocs;
@@ -216,7 +223,8 @@ bool add_axis(ozfft_plan_s *p, const AxisDesc &a, int axis, MatMap &mats, std::v
     g1.ns = pp;
     if (!a.contiguous) {
         const long long I = a.inner;
-        g1.nb = g2.nb = (int)(I / 32); g1.no = g2.no = (int)a.outer;
+        g1.nb = g2.nb = (int)((I + 31) / 32); g1.no = g2.no = (int)a.outer;
+        g1.ncols = g2.ncols = (int)I;
         g1.ib = 32; g1.is = I; g1.io = a.N * I;
         g1.lane = 1; g1.ji = pp * I; g1.ko = pp * I; g1.order = 0;
         g2.ib = 32; g2.is = pp * I; g2.io = a.N * I;
@@ -224,11 +232,12 @@ bool add_axis(ozfft_plan_s *p, const AxisDesc &a, int axis, MatMap &mats, std::v
         g2.lane = 1; g2.ji = I; g2.ko = 32 * I; g2.order = 0;
     } else {
         const long long Pn = a.outer;
-        g1.nb = g2.nb = (int)(Pn / 32); g1.no = g2.no = 1;
+        g1.nb = g2.nb = (int)((Pn + 31) / 32); g1.no = g2.no = 1;
+        g1.ncols = g2.ncols = (int)Pn;
         g1.ib = 32 * a.N; g1.is = 1; g1.io = 0;
         g1.lane = a.N; g1.ji = pp; g1.ko = pp; g1.order = 1;
         if (two && pp == 32) {  // N = 1024: a block is one pencil, lanes along j1 (adjacent elements): coalesced
-            g1.nb = (int)Pn; g1.ns = 1; g1.ib = a.N; g1.is = 0; g1.lane = 1; g1.order = 0;
+            g1.nb = (int)Pn; g1.ncols = 32 * (int)Pn; g1.ns = 1; g1.ib = a.N; g1.is = 0; g1.lane = 1; g1.order = 0;
         }
         g2.ib = 32 * a.N; g2.is = pp; g2.io = 0;
         g2.ob = 32 * a.N; g2.os = 1; g2.oo = 0;
@@ -301,9 +310,17 @@ ozfft_plan_s *make_plan(int nx, int ny, int nz, int sign, bool batched1d) {
         ok = cuda_ok(cudaMalloc(&p->work, (size_t)p->count * 16), "cudaMalloc(workspace)");
         if (ok) p->dev_bytes += (size_t)p->count * 16;
     }
+    // per plan, on the plan's device: kernel attributes and the constant bank (both are per-device state)
+    if (ok && p->variant == 0)
+        ok = cuda_ok(cudaFuncSetAttribute(stage_simt_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 32 * 32 * 16 + 12 * 32 * 32 * 4), "cudaFuncSetAttribute");
     if (ok && p->variant >= 1) ok = stage_tc_prepare(hc);  // uploads the constant bank both tensor-core kernels read
+    if (ok && p->variant == 1) stage_tc_occupancy(p->tc_per_sm);
     if (ok && p->variant == 2) ok = stage_bf_prepare();
     if (!ok && g_err.empty()) set_err("kernel attribute setup failed");
+    {
+        std::lock_guard<std::mutex> lk(g_plans_mu);
+        g_plans.insert(p);
+    }
     if (!ok) {
         std::string keep = g_err;
         ozfft_plan_destroy(p);
@@ -313,7 +330,10 @@ ozfft_plan_s *make_plan(int nx, int ny, int nz, int sign, bool batched1d) {
     return p;
 }
 
-bool valid(ozfft_plan p) { return p && p->magic == PLAN_MAGIC; }
+bool valid(ozfft_plan p) {
+    std::lock_guard<std::mutex> lk(g_plans_mu);
+    return p && g_plans.count(p) != 0;
+}
 
 int launch_stage(ozfft_plan p, const StageLaunch &s, const void *src, void *dst, cudaStream_t st) {
     const long long nt = (long long)s.g.nb * s.g.ns * s.g.no;
@@ -323,16 +343,11 @@ int launch_stage(ozfft_plan p, const StageLaunch &s, const void *src, void *dst,
         return OZFFT_ECUDA;
     }
     if (p->variant == 1) {
-        if (stage_tc_launch(s.g, src, dst, s.mat_tc, p->d_consts, st)) return OZFFT_OK;
+        if (stage_tc_launch(s.g, src, dst, s.mat_tc, p->sms, p->tc_per_sm, st)) return OZFFT_OK;
         set_err(std::string("stage_tc_kernel launch: ") + cudaGetErrorString(cudaGetLastError()));
         return OZFFT_ECUDA;
     }
     const size_t sm = (size_t)s.g.K * 32 * 16 + (size_t)12 * s.g.K * 32 * 4;
-    static bool attr = false;
-    if (!attr) {
-        cudaFuncSetAttribute(stage_simt_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 32 * 32 * 16 + 12 * 32 * 32 * 4);
-        attr = true;
-    }
     stage_simt_kernel<<<(unsigned)nt, SIMT_THREADS, sm, st>>>(s.g, (const ulonglong2 *)src, (ulonglong2 *)dst, s.mat_simt, p->d_consts);
     return cuda_ok(cudaGetLastError(), "stage_simt_kernel launch") ? OZFFT_OK : OZFFT_ECUDA;
 }
@@ -367,16 +382,12 @@ ozfft_plan ozfft_plan_create(int nx, int ny, int nz, int sign) {
         set_err("sizes must be powers of two in [2, 1024]");
         return nullptr;
     }
-    if (nz % 32 || ((long long)nx * ny) % 32) {
-        set_err("unsupported shape: nz and nx*ny must be multiples of 32 (tile width)");
-        return nullptr;
-    }
     return make_plan(nx, ny, nz, sign, false);
 }
 
 ozfft_plan ozfft_plan_create_1d(int n, int batch, int sign) {
-    if (!is_pow2(n) || n > 1024 || batch < 32 || batch % 32) {
-        set_err("n must be a power of two in [2, 1024] and batch a positive multiple of 32");
+    if (!is_pow2(n) || n > 1024 || batch < 1 || (long long)n * batch > (1ll << 30)) {
+        set_err("n must be a power of two in [2, 1024], batch >= 1 and n * batch <= 2^30 elements");
         return nullptr;
     }
     return make_plan(batch, 1, n, sign, true);
@@ -399,7 +410,7 @@ int ozfft_exec_axis(ozfft_plan p, int axis, const void *in, void *out, void *str
 }
 
 // pipelined host-buffer transform of a 3-D plan: H2D slab s || z,y passes of slab s-1;  x pass of chunk c || D2H of chunk c-1
-static int exec_host_pipelined(ozfft_plan p, const char *hin, char *hout, cudaStream_t st) {
+static int exec_host_pipelined_body(ozfft_plan p, const char *hin, char *hout, cudaStream_t st) {
     const long long nx = p->nx, ny = p->ny, nz = p->nz;
     const long long xs = nx / PIPE, yc = ny / PIPE;
     const size_t slab_elems = (size_t)(xs * ny * nz), slab_bytes = slab_elems * 16;
@@ -407,23 +418,22 @@ static int exec_host_pipelined(ozfft_plan p, const char *hin, char *hout, cudaSt
         if (!cuda_ok(cudaStreamCreateWithFlags(&p->s_in, cudaStreamNonBlocking), "cudaStreamCreate") ||
             !cuda_ok(cudaStreamCreateWithFlags(&p->s_out, cudaStreamNonBlocking), "cudaStreamCreate")) return OZFFT_ECUDA;
         for (int i = 0; i < PIPE; i++) {
-            cudaEventCreateWithFlags(&p->ev_in[i], cudaEventDisableTiming);
-            cudaEventCreateWithFlags(&p->ev_out[i], cudaEventDisableTiming);
+            if (!cuda_ok(cudaEventCreateWithFlags(&p->ev_in[i], cudaEventDisableTiming), "cudaEventCreate") ||
+                !cuda_ok(cudaEventCreateWithFlags(&p->ev_out[i], cudaEventDisableTiming), "cudaEventCreate")) return OZFFT_ECUDA;
         }
-        cudaEventCreateWithFlags(&p->ev_start, cudaEventDisableTiming);
+        if (!cuda_ok(cudaEventCreateWithFlags(&p->ev_start, cudaEventDisableTiming), "cudaEventCreate")) return OZFFT_ECUDA;
     }
     const size_t L = p->stages.size(), Lzy = p->slab_stages.size();
     auto buf_of = [&](size_t i) -> char * { return (char *)(((L - 1 - i) & 1) ? p->work : p->h_out); };  // as run_stages
     // copies start once earlier work on the caller's stream is done
-    cudaEventRecord(p->ev_start, st);
-    cudaStreamWaitEvent(p->s_in, p->ev_start, 0);
-    cudaStreamWaitEvent(p->s_out, p->ev_start, 0);
+    if (!cuda_ok(cudaEventRecord(p->ev_start, st), "cudaEventRecord") || !cuda_ok(cudaStreamWaitEvent(p->s_in, p->ev_start, 0), "cudaStreamWaitEvent") ||
+        !cuda_ok(cudaStreamWaitEvent(p->s_out, p->ev_start, 0), "cudaStreamWaitEvent")) return OZFFT_ECUDA;
     for (int s = 0; s < PIPE; s++) {
         if (!cuda_ok(cudaMemcpyAsync((char *)p->h_in + s * slab_bytes, hin + s * slab_bytes, slab_bytes, cudaMemcpyHostToDevice, p->s_in), "H2D slab")) return OZFFT_ECUDA;
-        cudaEventRecord(p->ev_in[s], p->s_in);
+        if (!cuda_ok(cudaEventRecord(p->ev_in[s], p->s_in), "cudaEventRecord")) return OZFFT_ECUDA;
     }
     for (int s = 0; s < PIPE; s++) {  // z and y passes of slab s
-        cudaStreamWaitEvent(st, p->ev_in[s], 0);
+        if (!cuda_ok(cudaStreamWaitEvent(st, p->ev_in[s], 0), "cudaStreamWaitEvent")) return OZFFT_ECUDA;
         const char *src = (const char *)p->h_in + s * slab_bytes;
         for (size_t i = 0; i < Lzy; i++) {
             char *dst = buf_of(i) + s * slab_bytes;
@@ -438,18 +448,32 @@ static int exec_host_pipelined(ozfft_plan p, const char *hin, char *hout, cudaSt
         for (size_t i = Lzy; i < L; i++) {
             StageLaunch sl = p->stages[i];
             sl.g.nb = (int)(yc * nz / 32);
+            sl.g.ncols = (int)(yc * nz);
             char *dst = buf_of(i) + off;
             int rc = launch_stage(p, sl, src, dst, st);
             if (rc) return rc;
             src = dst;
         }
-        cudaEventRecord(p->ev_out[c], st);
-        cudaStreamWaitEvent(p->s_out, p->ev_out[c], 0);
+        if (!cuda_ok(cudaEventRecord(p->ev_out[c], st), "cudaEventRecord") || !cuda_ok(cudaStreamWaitEvent(p->s_out, p->ev_out[c], 0), "cudaStreamWaitEvent")) return OZFFT_ECUDA;
         if (!cuda_ok(cudaMemcpy2DAsync(hout + off, (size_t)(ny * nz) * 16, (char *)p->h_out + off, (size_t)(ny * nz) * 16,
                                        (size_t)(yc * nz) * 16, (size_t)nx, cudaMemcpyDeviceToHost, p->s_out), "D2H chunk")) return OZFFT_ECUDA;
     }
     if (!cuda_ok(cudaStreamSynchronize(p->s_out), "cudaStreamSynchronize")) return OZFFT_ECUDA;
     return cuda_ok(cudaStreamSynchronize(st), "cudaStreamSynchronize") ? OZFFT_OK : OZFFT_ECUDA;
+}
+
+// On any failure the copies already queued on the plan's streams still touch the caller's host buffers and the plan's
+// staging memory: drain all three streams before reporting the error.
+static int exec_host_pipelined(ozfft_plan p, const char *hin, char *hout, cudaStream_t st) {
+    const int rc = exec_host_pipelined_body(p, hin, hout, st);
+    if (rc != OZFFT_OK) {
+        const std::string keep = g_err;
+        if (p->s_in) cudaStreamSynchronize(p->s_in);
+        if (p->s_out) cudaStreamSynchronize(p->s_out);
+        cudaStreamSynchronize(st);
+        set_err(keep);
+    }
+    return rc;
 }
 
 int ozfft_exec_host(ozfft_plan p, const void *host_in, void *host_out, void *stream) {
@@ -471,7 +495,10 @@ int ozfft_exec_host(ozfft_plan p, const void *host_in, void *host_out, void *str
 }
 
 void ozfft_plan_destroy(ozfft_plan p) {
-    if (!valid(p)) return;
+    {
+        std::lock_guard<std::mutex> lk(g_plans_mu);
+        if (!p || !g_plans.erase(p)) return;  // NULL, unknown or already destroyed: no-op
+    }
     for (void *d : p->dev_allocs) cudaFree(d);
     if (p->work) cudaFree(p->work);
     if (p->h_in) cudaFree(p->h_in);

@@ -13,6 +13,7 @@ namespace oz {
 struct StageGeom {
     int K;               // contraction length = number of outputs per column (2..32)
     int nb, ns, no;      // block grid
+    int ncols;           // columns along the b coordinate: column 32 b + lane exists iff it is < ncols (masked tail block)
     long long ib, is, io;  // input base strides per block coordinate
     long long ob, os, oo;  // output base strides
     long long lane;      // stride between the 32 columns of a block (same for input and output)

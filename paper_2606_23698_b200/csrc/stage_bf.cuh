@@ -282,7 +282,7 @@ __global__ void __launch_bounds__(BF_THREADS, 1) stage_bf_kernel(StageGeom g, co
             int tb, ts, to;
             tile_coords_pow2(g, tile, lg_nbt, lg_ns, tb, ts, to);
             const int blk = 4 * tb + (c >> 5);
-            const bool valid = blk < g.nb;
+            const bool valid = blk * 32 + (c & 31) < g.ncols;
             const uint4 *src = in + ((long long)blk * g.ib + (long long)ts * g.is + (long long)to * g.io + (long long)(c & 31) * g.lane + (long long)par * g.ji);
             const long long jstep = 2 * g.ji;
             // a2: column exponent = max of the 11-bit exponent fields (integer compare on the high words)
@@ -366,7 +366,7 @@ __global__ void __launch_bounds__(BF_THREADS, 1) stage_bf_kernel(StageGeom g, co
             int tb, ts, to;
             tile_coords_pow2(g, tile, lg_nbt, lg_ns, tb, ts, to);
             const int blk = 4 * tb + (row >> 5);
-            const bool valid = blk < g.nb;
+            const bool valid = blk * 32 + (row & 31) < g.ncols;
             uint4 *dstp = out + ((long long)blk * g.ob + (long long)ts * g.os + (long long)to * g.oo + (long long)(row & 31) * g.lane);
             const uint4 *ct = ctab + (size_t)(g.matsel ? ts : 0) * K;
             bf_wait(&a_full[0], it & 1);  // the column exponents of this tile are published (s_T is double buffered: the

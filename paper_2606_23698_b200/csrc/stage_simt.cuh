@@ -34,10 +34,11 @@ __global__ void __launch_bounds__(SIMT_THREADS) stage_simt_kernel(StageGeom g, c
     const long long ibase = tb * g.ib + ts * g.is + to * g.io + lane * g.lane;
     const long long obase = tb * g.ob + ts * g.os + to * g.oo + lane * g.lane;
     const int mid = g.matsel ? ts : 0;
+    const bool valid = tb * 32 + lane < g.ncols;  // masked tail block
 
     // ---- load + column exponent (a1, a2)
     for (int j = grp; j < K; j += SIMT_KG) {
-        const ulonglong2 v = in[ibase + j * g.ji];
+        const ulonglong2 v = valid ? in[ibase + j * g.ji] : make_ulonglong2(0, 0);
         s_bits[j * 32 + lane] = v;
         int T, cls, fl = 0, tm = -100000;
         cls = classify_top(v.x, T);
@@ -93,7 +94,7 @@ __global__ void __launch_bounds__(SIMT_THREADS) stage_simt_kernel(StageGeom g, c
             y.x = pack_rne(crt_centre(vr, c), gexp);
             y.y = pack_rne(crt_centre(vi, c), gexp);
         }
-        out[obase + k * g.ko] = y;
+        if (valid) out[obase + k * g.ko] = y;
     }
 }
 

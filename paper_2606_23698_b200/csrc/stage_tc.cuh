@@ -24,11 +24,8 @@
 
 namespace oz {
 
-#ifndef TC_Q32
-#define TC_Q32 4
-#endif
 // threads per CTA = 128 * Q: Q thread groups share each MMA row and split its contraction elements / outputs
-__host__ __device__ constexpr int tc_q(int KP) { return KP >= 32 ? TC_Q32 : 4; }
+__host__ __device__ constexpr int tc_q(int KP) { return 4; }
 // TMEM columns: [0,256) stage accumulators (2 pairs x 2 x 64); the Phase-A sums of batch b reuse [128 b, 128 b + 128)
 __host__ __device__ constexpr int tc_tmem_cols(int KP) { return KP >= 32 ? 512 : 256; }
 
@@ -117,7 +114,7 @@ __global__ void __launch_bounds__(128 * tc_q(KP), KP >= 32 ? 1 : 2) stage_tc_ker
         int tb, ts, to;
         tile_coords_pow2(g, t, lg_nbt, lg_ns, tb, ts, to);
         const int blk = 2 * tb + (col >> 5);
-        valid = blk < g.nb;
+        valid = blk * 32 + (col & 31) < g.ncols;
         ib = (uint32_t)blk * (uint32_t)g.ib + (uint32_t)ts * (uint32_t)g.is + (uint32_t)to * (uint32_t)g.io + (uint32_t)(col & 31) * (uint32_t)g.lane;
         ob = (uint32_t)blk * (uint32_t)g.ob + (uint32_t)ts * (uint32_t)g.os + (uint32_t)to * (uint32_t)g.oo + (uint32_t)(col & 31) * (uint32_t)g.lane;
         mb = mat + (size_t)(g.matsel ? ts : 0) * 12 * MB;
@@ -374,37 +371,38 @@ inline bool stage_tc_prepare(const DevConsts &hc) {
     return e == cudaSuccess;
 }
 
-template <int KP>
-inline bool stage_tc_launch_kp(const StageGeom &g, const uint64_t *in, ulonglong2 *out, const uint8_t *mat, long long nt, int sms, cudaStream_t st) {
-    static int per_sm = 0;  // resident CTAs per SM for this instantiation (persistent grid = sms * per_sm)
-    if (!per_sm) {
-        cudaFuncAttributes fa;
-        int dev = 0, smem_sm = 0, regs_sm = 0;
-        cudaGetDevice(&dev);
-        cudaDeviceGetAttribute(&smem_sm, cudaDevAttrMaxSharedMemoryPerMultiprocessor, dev);
-        cudaDeviceGetAttribute(&regs_sm, cudaDevAttrMaxRegistersPerMultiprocessor, dev);
-        per_sm = 1;
-        if (cudaFuncGetAttributes(&fa, stage_tc_kernel<KP>) == cudaSuccess) {
-            const int by_smem = smem_sm / (int)(tc_smem_bytes(KP) + fa.sharedSizeBytes + 1024);
-            const int by_regs = regs_sm / (((fa.numRegs + 7) & ~7) * 128 * tc_q(KP));
-            per_sm = by_smem < by_regs ? by_smem : by_regs;
-        }
-        if (per_sm < 1) per_sm = 1;
-        if (per_sm > 512 / tc_tmem_cols(KP)) per_sm = 512 / tc_tmem_cols(KP);  // TMEM columns
+// resident CTAs per SM of one instantiation on the current device (persistent grid = SMs x this)
+template <int KP> inline int stage_tc_per_sm() {
+    cudaFuncAttributes fa;
+    int dev = 0, smem_sm = 0, regs_sm = 0, per_sm = 1;
+    cudaGetDevice(&dev);
+    cudaDeviceGetAttribute(&smem_sm, cudaDevAttrMaxSharedMemoryPerMultiprocessor, dev);
+    cudaDeviceGetAttribute(&regs_sm, cudaDevAttrMaxRegistersPerMultiprocessor, dev);
+    if (cudaFuncGetAttributes(&fa, stage_tc_kernel<KP>) == cudaSuccess) {
+        const int by_smem = smem_sm / (int)(tc_smem_bytes(KP) + fa.sharedSizeBytes + 1024);
+        const int by_regs = regs_sm / (((fa.numRegs + 7) & ~7) * 128 * tc_q(KP));
+        per_sm = by_smem < by_regs ? by_smem : by_regs;
     }
+    if (per_sm < 1) per_sm = 1;
+    if (per_sm > 512 / tc_tmem_cols(KP)) per_sm = 512 / tc_tmem_cols(KP);  // TMEM columns
+    return per_sm;
+}
+// per_sm[0..2]: KP = 8, 16, 32 (kept in the plan: per-device state)
+inline void stage_tc_occupancy(int *per_sm) {
+    per_sm[0] = stage_tc_per_sm<8>();
+    per_sm[1] = stage_tc_per_sm<16>();
+    per_sm[2] = stage_tc_per_sm<32>();
+}
+
+template <int KP>
+inline bool stage_tc_launch_kp(const StageGeom &g, const uint64_t *in, ulonglong2 *out, const uint8_t *mat, long long nt, int sms, int per_sm, cudaStream_t st) {
     const long long cap = (long long)sms * per_sm;
     const unsigned grid = (unsigned)(nt < cap ? nt : cap);
     stage_tc_kernel<KP><<<grid, 128 * tc_q(KP), tc_smem_bytes(KP), st>>>(g, in, out, mat, nt);
     return cudaGetLastError() == cudaSuccess;
 }
 
-inline bool stage_tc_launch(const StageGeom &g, const void *src, void *dst, const uint8_t *mat, const DevConsts *, cudaStream_t st) {
-    static int sms = 0;
-    if (!sms) {
-        int dev = 0;
-        cudaGetDevice(&dev);
-        cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
-    }
+inline bool stage_tc_launch(const StageGeom &g, const void *src, void *dst, const uint8_t *mat, int sms, const int *per_sm, cudaStream_t st) {
     const int KP = tc_pad(g.K);
     int nbt = 1;
     while (nbt < (g.nb + 1) / 2) nbt <<= 1;  // rounded up to a power of two: shifts instead of divisions on the device
@@ -413,9 +411,9 @@ inline bool stage_tc_launch(const StageGeom &g, const void *src, void *dst, cons
     if (nt >= (1ll << 31)) return false;
     const uint64_t *in = (const uint64_t *)src;
     ulonglong2 *out = (ulonglong2 *)dst;
-    if (KP == 32) return stage_tc_launch_kp<32>(g, in, out, mat, nt, sms, st);
-    if (KP == 16) return stage_tc_launch_kp<16>(g, in, out, mat, nt, sms, st);
-    return stage_tc_launch_kp<8>(g, in, out, mat, nt, sms, st);
+    if (KP == 32) return stage_tc_launch_kp<32>(g, in, out, mat, nt, sms, per_sm[2], st);
+    if (KP == 16) return stage_tc_launch_kp<16>(g, in, out, mat, nt, sms, per_sm[1], st);
+    return stage_tc_launch_kp<8>(g, in, out, mat, nt, sms, per_sm[0], st);
 }
 
 }  // namespace oz

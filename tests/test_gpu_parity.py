@@ -158,12 +158,71 @@ def test_bad_arguments():
     with pytest.raises(RuntimeError):
         ozfft.Plan(32, 32, 48)
     with pytest.raises(RuntimeError):
-        ozfft.Plan(32, 32, 16)  # nz not a multiple of the tile width
+        ozfft.Plan(32, 32, 2048)  # beyond the K <= 32 capacity budget
     plan = ozfft.Plan(32, 32, 32)
     x = torch.zeros(32 ** 3, dtype=torch.complex128, device="cuda")
     assert ozfft.lib().ozfft_exec(plan.h, x.data_ptr(), x.data_ptr(), None) == 1  # in == out
     assert ozfft.lib().ozfft_exec(plan.h, x.data_ptr() + 8, x.data_ptr(), None) == 1  # misaligned
     plan.destroy()
+
+
+@pytest.mark.parametrize("shape", [(16, 16, 16), (8, 8, 32), (2, 2, 2), (4, 64, 8), (2, 1024, 4)])
+def test_small_shapes_masked_tail_tiles(O, shape):
+    """every power-of-two size in [2, 1024] per axis is accepted: blocks with fewer than 32 columns and
+    tiles with missing blocks are masked, not rejected"""
+    from paper_2606_23698_b200 import inputs
+    x = inputs.uniform_pm1(shape, 17)
+    _assert_bit_exact(_run3d(x), O.fft3d(x, -1, route=0)[0])
+    _assert_bit_exact(_run3d(x, +1), O.fft3d(x, +1, route=0)[0])
+
+
+@pytest.mark.parametrize("n,batch", [(1024, 1), (64, 5), (8, 33), (512, 100), (2, 7)])
+def test_batched_1d_any_batch(O, n, batch):
+    from paper_2606_23698_b200 import inputs
+    x = inputs.normal((batch, n), 19)
+    _assert_bit_exact(_run1d(x), O.fft1d(x, -1, route=0)[0])
+
+
+def test_plan_lifetime_and_threads(O, variant):
+    """a destroyed handle is refused without touching freed memory; destroying twice is a no-op; two plans created and
+    executed from two host threads (each on its own stream) give the oracle's bits"""
+    if variant == "simt":
+        pytest.skip("host-side logic; run on the tensor-core kernels")
+    import threading
+    torch = _torch()
+    from paper_2606_23698_b200 import inputs, ozfft
+    plan = ozfft.Plan(32, 32, 32)
+    h = plan.h
+    x = torch.zeros(32 ** 3, dtype=torch.complex128, device="cuda")
+    y = torch.empty_like(x)
+    assert ozfft.lib().ozfft_exec(h, x.data_ptr(), y.data_ptr(), None) == 0
+    torch.cuda.synchronize()
+    ozfft.lib().ozfft_plan_destroy(h)
+    ozfft.lib().ozfft_plan_destroy(h)  # second destroy: no-op
+    assert ozfft.lib().ozfft_exec(h, x.data_ptr(), y.data_ptr(), None) == 1  # OZFFT_EINVAL
+    assert ozfft.lib().ozfft_plan_num_launches(h) == -1
+    plan.h = None
+    res = {}
+
+    def work(i, shape, sign):
+        xx = inputs.uniform_pm1(shape, 30 + i)
+        st = torch.cuda.Stream()
+        with torch.cuda.stream(st):
+            p = ozfft.Plan(*shape, sign=sign)
+            d = torch.from_numpy(xx).cuda()
+            out = p.exec(d, stream=st.cuda_stream)
+            st.synchronize()
+            res[i] = (xx, sign, out.cpu().numpy())
+            p.destroy()
+
+    ts = [threading.Thread(target=work, args=(0, (32, 64, 32), -1)), threading.Thread(target=work, args=(1, (64, 32, 128), +1))]
+    for t in ts:
+        t.start()
+    for t in ts:
+        t.join()
+    for i in (0, 1):
+        xx, sign, got = res[i]
+        _assert_bit_exact(got, O.fft3d(xx, sign, route=0)[0])
 
 
 def test_exec_host_pipelined_path(O, variant):

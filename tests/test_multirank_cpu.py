@@ -47,3 +47,25 @@ def test_reference_arm_only_rank0_prints(capsys, monkeypatch):
     monkeypatch.setenv("RANK", "1")
     bench.run_reference(type("A", (), {"size": 32, "gpus": 2, "steps": 1, "warmup": 0})())
     assert capsys.readouterr().out == ""
+
+
+def test_bench_gpus_flag_spawns_that_many_ranks():
+    """`python bench.py --gpus 2` with no WORLD_SIZE in the environment must run two ranks (it re-launches itself under
+    torch.distributed.run); the dry run goes through the same spawn and MAX-over-ranks code on gloo."""
+    import json
+    import subprocess
+    env = {k: v for k, v in os.environ.items() if k not in ("WORLD_SIZE", "RANK", "LOCAL_RANK", "MASTER_ADDR", "MASTER_PORT")}
+    out = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--gpus", "2", "--dry-run"], env=env, capture_output=True,
+                         text=True, timeout=300)
+    assert out.returncode == 0, out.stderr[-2000:]
+    lines = [json.loads(l) for l in out.stdout.splitlines() if l.startswith("{")]
+    assert lines == [{"dry_run": True, "n_gpus": 2, "max_rank_seen": 1.0}]
+
+
+def test_bench_refuses_a_world_size_that_contradicts_gpus(monkeypatch):
+    sys.path.insert(0, ROOT)
+    import bench
+    import pytest
+    monkeypatch.setenv("WORLD_SIZE", "1")
+    with pytest.raises(SystemExit):
+        bench.run_ours(type("A", (), {"size": 32, "gpus": 2, "steps": 1, "warmup": 0, "dry_run": True, "no_cpu": True})())
