@@ -138,17 +138,21 @@ template <int K> __host__ __device__ constexpr size_t bf_smem_bytes() {
     return (size_t)bf_aset_bytes(K) + (size_t)BF_NSLOT * bf_slot_bytes(K) + BF_PA_BYTES;
 }
 
-// bounded wait: a pipeline bug must not hang the GPU (traps after 2^22 failed polls of up to 1 ms each)
-__device__ __forceinline__ void bf_wait(uint64_t *bar, uint32_t parity) {
+// bounded wait: a pipeline bug must not hang the GPU (traps after 2^26 failed polls).  The poll loop is four
+// instructions; BACKOFF > 0 parks the warp that many nanoseconds between polls (roles with slack: their polls would
+// otherwise take issue slots from the working warps).
+template <int BACKOFF> __device__ __forceinline__ void bf_wait_t(uint64_t *bar, uint32_t parity) {
     const uint32_t a = smem_u32(bar);
     uint32_t done, spins = 0;
     do {
         // the suspend-time hint lets the hardware park the warp instead of re-issuing the poll
         asm volatile("{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2, %3;\n\tselp.u32 %0, 1, 0, p;\n\t}"
                      : "=r"(done) : "r"(a), "r"(parity), "r"(1000000u) : "memory");
-        if (!done && ++spins > (1u << 22)) __trap();
+        if (!done && ++spins > (1u << 26)) __trap();
     } while (!done);
 }
+__device__ __forceinline__ void bf_wait(uint64_t *bar, uint32_t parity) { bf_wait_t<0>(bar, parity); }
+__device__ __forceinline__ void bf_wait_slack(uint64_t *bar, uint32_t parity) { bf_wait_t<0>(bar, parity); }
 
 // append the 7 bytes of w = (hi:lo) (hi < 2^24) at byte position 7 e of a little-endian word array; e is a
 // compile-time constant after unrolling, so every index and shift folds
@@ -309,7 +313,7 @@ __global__ void __launch_bounds__(BF_THREADS, 1) stage_bf_kernel(StageGeom g, co
                 if (ef == 0 && tm > -100000) { flag = 1; Tmax = tm; }
             }
             // the previous tile's operand must have been copied to TMEM before the shared copy is overwritten
-            if (it >= 1) bf_wait(&a_empty[0], (it - 1) & 1);
+            if (it >= 1) bf_wait_slack(&a_empty[0], (it - 1) & 1);
             if (par == 0) { s_T[buf][c] = Tmax; s_flag[buf][c] = flag; }
             // a3: quantise, offset by 2^53, split into bytes; planes XI (0), XR (1), NXI (2)
             uint32_t wr[NW + 2], wi[NW + 2], wn[NW + 2];
@@ -351,7 +355,7 @@ __global__ void __launch_bounds__(BF_THREADS, 1) stage_bf_kernel(StageGeom g, co
                 }
             // every epilogue warp must have observed the a_full phase of tile it-1 (and read its exponents) before
             // this tile's phase may complete: a waiter that falls two phases behind would wait forever
-            if (it >= 1) bf_wait(&e_start[0], (it - 1) & 1);
+            if (it >= 1) bf_wait_slack(&e_start[0], (it - 1) & 1);
             fence_async_smem();
             __syncwarp();
             if (lane == 0) mbar_arrive(&a_full[0]);
@@ -360,7 +364,8 @@ __global__ void __launch_bounds__(BF_THREADS, 1) stage_bf_kernel(StageGeom g, co
         // ------------------------------------------------ epilogue: thread = data column (TMEM lane), both parts
         const int qd = (warp - 12) >> 2, row = (warp & 3) * 32 + lane;
         const uint32_t lane_taddr = tmem + ((uint32_t)((warp & 3) * 32) << 16);
-        uint32_t it = 0, u = 0;
+        uint32_t it = 0, nu = 0;  // tiles seen, units this group has consumed
+        int turn = qd;            // units to skip until the next one of this group (units go round-robin over the 3 groups)
         for (long long tile = blockIdx.x; tile < ntiles; tile += gridDim.x, it++) {
             const uint32_t buf = it & 1;
             int tb, ts, to;
@@ -369,21 +374,23 @@ __global__ void __launch_bounds__(BF_THREADS, 1) stage_bf_kernel(StageGeom g, co
             const bool valid = blk * 32 + (row & 31) < g.ncols;
             uint4 *dstp = out + ((long long)blk * g.ob + (long long)ts * g.os + (long long)to * g.oo + (long long)(row & 31) * g.lane);
             const uint4 *ct = ctab + (size_t)(g.matsel ? ts : 0) * K;
-            bf_wait(&a_full[0], it & 1);  // the column exponents of this tile are published (s_T is double buffered: the
+            bf_wait_slack(&a_full[0], it & 1);  // the column exponents of this tile are published (s_T is double buffered: the
             const int Tmax = s_T[buf][row], flag = s_flag[buf][row];  // deconstruction runs at most one tile ahead)
             __syncwarp();
             if (lane == 0) mbar_arrive(&e_start[0]);
             const int gexp = 53 + 52 - Tmax;
+            const long long hko = (long long)H * g.ko;  // output k + H sits this far from output k
 #pragma unroll 1
             for (int ch = 0; ch < NCH; ch++)
 #pragma unroll 1
-                for (int gg = 0; gg < 2; gg++, u++) {
-                    if ((int)(u % 3) != qd) continue;
+                for (int gg = 0; gg < 2; gg++) {
+                    if (turn) { turn--; continue; }
+                    turn = 2;
                     const int kp = 2 * ch + gg;
                     uint4 cc[2];
                     cc[0] = __ldg(ct + (kp < H ? kp : 0));
                     cc[1] = __ldg(ct + (kp < H ? kp + H : 0));
-                    bf_wait(&pa_full[qd], (u / 3) & 1);
+                    bf_wait_slack(&pa_full[qd], nu & 1);
                     tc_fence_after();
                     uint32_t E[4][5];  // [part*2 + o]
 #pragma unroll
@@ -396,24 +403,27 @@ __global__ void __launch_bounds__(BF_THREADS, 1) stage_bf_kernel(StageGeom g, co
                     tc_fence_before();
                     __syncwarp();
                     if (lane == 0) mbar_arrive(&pa_empty[qd]);
-                    if (kp >= H) continue;
+                    nu++;
+                    if (kp >= H || !valid) continue;
+                    uint4 *dk = dstp + (long long)kp * g.ko;
+                    if (flag == 1) {  // the usual column: finite, not all zero
 #pragma unroll
-                    for (int o = 0; o < 2; o++) {
-                        const int k = kp + o * H;
-                        uint64_t y[2];
+                        for (int o = 0; o < 2; o++) {
+                            uint64_t y[2];
 #pragma unroll
-                        for (int P = 0; P < 2; P++) {
-                            if (flag & 2) y[P] = 0x7FF8000000000000ull;
-                            else if (flag == 0) y[P] = 0;
-                            else {
+                            for (int P = 0; P < 2; P++) {
                                 const uint32_t *e = E[P * 2 + o];
                                 uint32_t r[4], r2[4];
-                                crt_from_E(e[0], e[1], e[2], e[3], e[4], r);
-                                sub128(r2, r[0], r[1], r[2], r[3], cc[o].x, cc[o].y, cc[o].z, cc[o].w);
-                                y[P] = pack_limbs(r2, gexp);
+                                crt_from_E(e[0], e[1], e[2], e[3], e[4], r);                        // a8: lift, two-sided centring
+                                sub128(r2, r[0], r[1], r[2], r[3], cc[o].x, cc[o].y, cc[o].z, cc[o].w);  // minus the offset constant
+                                y[P] = pack_limbs(r2, gexp);                                        // a9: one rounding to fp64
                             }
+                            dk[o * hko] = make_uint4((uint32_t)y[0], (uint32_t)(y[0] >> 32), (uint32_t)y[1], (uint32_t)(y[1] >> 32));  // a12
                         }
-                        if (valid) dstp[(long long)k * g.ko] = make_uint4((uint32_t)y[0], (uint32_t)(y[0] >> 32), (uint32_t)y[1], (uint32_t)(y[1] >> 32));
+                    } else {  // all-zero column -> +0, non-finite column -> NaN (reading S18)
+                        const uint32_t hi = (flag & 2) ? 0x7FF80000u : 0u;
+                        dk[0] = make_uint4(0, hi, 0, hi);
+                        dk[hko] = make_uint4(0, hi, 0, hi);
                     }
                 }
         }
