@@ -28,11 +28,16 @@ struct DevConsts {
     uint32_t m2m2[12];   // 2m in both half-words
     uint32_t off30[12];  // smallest multiple of m >= 2^30: makes the signed plane sum of the deconstruction positive
     uint32_t phaseA[128];  // Phase-A constant matrix: 16 slice rows x 32 bytes in MMA operand order
+    // ablation rungs only (PAPER.md:260-273 Garner, 340-345 naive fp64 Phase B)
+    uint16_t gprod[12][12];  // gprod[j][k] = (m_0 ... m_{j-1}) mod m_k  (Eq. 10)
+    uint16_t ginv[12];       // (m_0 ... m_{k-1})^-1 mod m_k
+    uint8_t uslice[12][16];  // byte s of u_k (Eq. 18)
 };
 
 // the same constants in the constant bank (uniform operands, no shared-memory loads); set by stage_tc_prepare
 __constant__ DevConsts kc;
 
+// [ledger: a2 column exponent]
 // value class of an fp64 bit pattern; T = floor(log2 |x|) for finite nonzero x
 enum { CLS_ZERO = 0, CLS_FINITE = 1, CLS_NONFINITE = 2 };
 
@@ -47,6 +52,7 @@ __device__ __forceinline__ int classify_top(uint64_t b, int &T) {
     return CLS_FINITE;
 }
 
+// [ledger: a3 deconstruction: quantise, offset, byte planes]
 // |RNE(x * 2^(52 - Tmax))| as an integer < 2^53; sign returned separately (bit 63 of b)
 __device__ __forceinline__ uint64_t quantise_mag(uint64_t b, int Tmax) {
     const int ef = (int)((b >> 52) & 0x7FF);
@@ -83,6 +89,7 @@ __device__ __forceinline__ uint64_t quantise_mag_fast(uint64_t b, int Tmax) {
     return quantise_mag_slow(b, Tmax);  // more than 2^32 below the column maximum
 }
 
+// [ledger: a3/a5 residues: plane dot, Barrett, digit packing]
 // r in [0, 2^32) -> r mod m by Barrett with mu = floor(2^32/m): one multiply-high, one conditional subtract
 __device__ __forceinline__ uint32_t barrett(uint32_t r, uint32_t m, uint32_t mu) {
     uint32_t q = __umulhi(r, mu);
@@ -111,6 +118,7 @@ __device__ __forceinline__ uint32_t residue53(uint64_t a, int i, const DevConsts
     return barrett(r, c.m[i], c.mu[i]);
 }
 
+// [ledger: a9 pack]
 typedef unsigned __int128 u128;
 typedef __int128 i128;
 
@@ -156,6 +164,7 @@ __device__ __noinline__ uint64_t pack_rne_slow(uint32_t r0, uint32_t r1, uint32_
     return pack_rne((i128)(((u128)r3 << 96) | ((u128)r2 << 64) | ((u128)r1 << 32) | r0), g);
 }
 
+// [ledger: a8 lift: quotient, E - zM, centring, offset constant]
 // Exact CRT of 12 canonical residues to the centred representative in [-M/2, M/2)
 // (PAPER.md:316-329 direct CRT with idempotents; 370-373 fractional lift and two-sided correction).
 // Plain multiword form used by the SIMT reference kernel: all sums are taken mod 2^128, which is exact
@@ -188,6 +197,7 @@ __device__ __forceinline__ void sub128(uint32_t *r, uint32_t a0, uint32_t a1, ui
         : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3])
         : "r"(a0), "r"(a1), "r"(a2), "r"(a3), "r"(b0), "r"(b1), "r"(b2), "r"(b3));
 }
+// [ledger: a9 pack]
 // |x| of a two's-complement 128-bit value: (x ^ sm) + (sm & 1) with sm = sign mask, one carry chain
 __device__ __forceinline__ void abs128(uint32_t *a, const uint32_t *x, uint32_t sm) {
     asm("add.cc.u32 %0, %4, %8;\n\taddc.cc.u32 %1, %5, 0;\n\taddc.cc.u32 %2, %6, 0;\n\taddc.u32 %3, %7, 0;"
@@ -195,6 +205,7 @@ __device__ __forceinline__ void abs128(uint32_t *a, const uint32_t *x, uint32_t 
         : "r"(x[0] ^ sm), "r"(x[1] ^ sm), "r"(x[2] ^ sm), "r"(x[3] ^ sm), "r"(sm & 1));
 }
 
+// [ledger: a8 lift: quotient, E - zM, centring, offset constant]
 // Direct CRT E = sum_k v_k u_k (Eq. 17) on residues that need not be canonical (v_k < 2^13, any
 // representative: m_k u_k == 0 mod M), quotient zhat = round(E/M) read off the top 30 bits of E (the lift of
 // PAPER.md:370 with the fraction taken from E itself), R = E - zhat M, two-sided centring.
@@ -227,6 +238,7 @@ __device__ __forceinline__ void crt_limbs(const uint32_t *v, uint32_t *r) {
     crt_from_E((uint32_t)a0, (uint32_t)a1, (uint32_t)a2, (uint32_t)a3, (uint32_t)(a3 >> 32), r);
 }
 
+// [ledger: a7 Phase B deposits (TMEM loads, slice sums -> E)]
 // Phase B (Alg. 2): deposit the 16 Phase-A slice sums P_s (each < 2^21) at byte offsets
 // 8s -- four 64-bit words of four slices each, one carry sweep -- giving E = sum_s P_s 256^s in 32-bit limbs.
 __device__ __forceinline__ void deposit_slices(const uint32_t *P, uint32_t *r) {
@@ -252,6 +264,7 @@ __device__ __forceinline__ void slices_to_E(const uint32_t *P, uint32_t *e) {
     e[0] = (uint32_t)w[0]; e[1] = (uint32_t)t1; e[2] = (uint32_t)t2; e[3] = (uint32_t)t3; e[4] = (uint32_t)(t3 >> 32);
 }
 
+// [ledger: a8 lift: quotient, E - zM, centring, offset constant]
 // lift and centring from the limbs of E (< 2^134): see crt_limbs
 __device__ __forceinline__ void crt_from_E(uint32_t e0, uint32_t e1, uint32_t e2, uint32_t e3, uint32_t e4, uint32_t *r) {
     const uint32_t T = __funnelshift_r(e3, e4, 8);  // E >> 104
@@ -268,6 +281,7 @@ __device__ __forceinline__ void crt_from_E(uint32_t e0, uint32_t e1, uint32_t e2
     }
 }
 
+// [ledger: a9 pack]
 // RNE_fp64(R * 2^-g) from two's-complement limbs (DESIGN.md A.6); normal-range results take the limb path,
 // zero / subnormal / overflowing ones the generic pack_rne.
 __device__ __forceinline__ uint64_t pack_limbs(const uint32_t *r, int g) {

@@ -57,7 +57,7 @@ struct ozfft_plan_s {
     uint32_t magic;
     int nx, ny, nz, sign;
     long long count;
-    int variant;  // 0 simt, 1 tensor-core (residue digits), 2 byte-fed tensor-core (default)
+    int variant;  // 0 simt, 1 tensor-core (residue digits), 2 byte-fed tensor-core (default), 3 / 4 ablations on the simt kernel
     int sms;      // SM count of the plan's device
     int tc_per_sm[3];  // resident CTAs per SM of the residue-digit kernel instantiations (per device)
     const void *pa_bf;  // Phase-A constant matrix of the byte-fed kernel
@@ -127,6 +127,16 @@ void fill_consts(DevConsts &c) {
                     pa[(kap / 16) * 256 + s * 16 + kap % 16] = b;
                 }
     }
+    for (int k = 0; k < R_MOD; k++) {  // ablation tables: Garner mixed-radix constants, idempotent byte slices
+        const int mk = kModuli[k];
+        long prod = 1 % mk;
+        for (int j = 0; j < R_MOD; j++) {
+            c.gprod[j][k] = (uint16_t)prod;  // product of the first j moduli, mod m_k
+            if (j == k) c.ginv[k] = (uint16_t)mod_inverse((int)prod, mk);
+            prod = (prod * (kModuli[j] % mk)) % mk;
+        }
+        for (int s = 0; s < 16; s++) c.uslice[k][s] = (uint8_t)(C.u[k] >> (8 * s));
+    }
     for (int l = 0; l < 4; l++) {
         c.M[l] = (uint32_t)(C.M >> (32 * l));
         c.Mh[l] = (uint32_t)(C.Mhalf >> (32 * l));
@@ -191,7 +201,7 @@ bool add_axis(ozfft_plan_s *p, const AxisDesc &a, int axis, MatMap &mats, std::v
         auto it = mats.find(key);
         if (it == mats.end()) {
             MatSet ms{};
-            if (p->variant == 0) {
+            if (p->variant == 0 || p->variant >= 3) {
                 ms.simt = build_mat_simt(p, K, fusedN);
                 if (!ms.simt) return false;
             } else if (p->variant == 1) {
@@ -257,6 +267,8 @@ int pick_variant() {
     const char *v = getenv("OZFFT_VARIANT");
     if (v && !strcmp(v, "simt")) return 0;
     if (v && !strcmp(v, "tc")) return 1;
+    if (v && !strcmp(v, "garner")) return 3;   // ablation: SIMT kernel with recursive Garner reconstruction
+    if (v && !strcmp(v, "fp64sum")) return 4;  // ablation: SIMT kernel with the naive fp64 Phase B (NOT exact, uses fp64)
     return 2;
 }
 
@@ -311,9 +323,13 @@ ozfft_plan_s *make_plan(int nx, int ny, int nz, int sign, bool batched1d) {
         if (ok) p->dev_bytes += (size_t)p->count * 16;
     }
     // per plan, on the plan's device: kernel attributes and the constant bank (both are per-device state)
-    if (ok && p->variant == 0)
-        ok = cuda_ok(cudaFuncSetAttribute(stage_simt_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 32 * 32 * 16 + 12 * 32 * 32 * 4), "cudaFuncSetAttribute");
-    if (ok && p->variant >= 1) ok = stage_tc_prepare(hc);  // uploads the constant bank both tensor-core kernels read
+    if (ok && (p->variant == 0 || p->variant >= 3)) {
+        const int sm = 32 * 32 * 16 + 12 * 32 * 32 * 4;
+        ok = cuda_ok(cudaFuncSetAttribute(stage_simt_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, sm), "cudaFuncSetAttribute") &&
+             cuda_ok(cudaFuncSetAttribute(stage_garner_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, sm), "cudaFuncSetAttribute") &&
+             cuda_ok(cudaFuncSetAttribute(stage_fp64sum_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, sm), "cudaFuncSetAttribute");
+    }
+    if (ok && (p->variant == 1 || p->variant == 2)) ok = stage_tc_prepare(hc);  // uploads the constant bank both tensor-core kernels read
     if (ok && p->variant == 1) stage_tc_occupancy(p->tc_per_sm);
     if (ok && p->variant == 2) ok = stage_bf_prepare();
     if (!ok && g_err.empty()) set_err("kernel attribute setup failed");
@@ -348,7 +364,9 @@ int launch_stage(ozfft_plan p, const StageLaunch &s, const void *src, void *dst,
         return OZFFT_ECUDA;
     }
     const size_t sm = (size_t)s.g.K * 32 * 16 + (size_t)12 * s.g.K * 32 * 4;
-    stage_simt_kernel<<<(unsigned)nt, SIMT_THREADS, sm, st>>>(s.g, (const ulonglong2 *)src, (ulonglong2 *)dst, s.mat_simt, p->d_consts);
+    if (p->variant == 3) stage_garner_kernel<<<(unsigned)nt, SIMT_THREADS, sm, st>>>(s.g, (const ulonglong2 *)src, (ulonglong2 *)dst, s.mat_simt, p->d_consts);
+    else if (p->variant == 4) stage_fp64sum_kernel<<<(unsigned)nt, SIMT_THREADS, sm, st>>>(s.g, (const ulonglong2 *)src, (ulonglong2 *)dst, s.mat_simt, p->d_consts);
+    else stage_simt_kernel<<<(unsigned)nt, SIMT_THREADS, sm, st>>>(s.g, (const ulonglong2 *)src, (ulonglong2 *)dst, s.mat_simt, p->d_consts);
     return cuda_ok(cudaGetLastError(), "stage_simt_kernel launch") ? OZFFT_OK : OZFFT_ECUDA;
 }
 

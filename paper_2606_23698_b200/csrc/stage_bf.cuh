@@ -138,6 +138,7 @@ template <int K> __host__ __device__ constexpr size_t bf_smem_bytes() {
     return (size_t)bf_aset_bytes(K) + (size_t)BF_NSLOT * bf_slot_bytes(K) + BF_PA_BYTES;
 }
 
+// [ledger: sync: mbarrier waits]
 // bounded wait: a pipeline bug must not hang the GPU (traps after 2^26 failed polls).  The poll loop is four
 // instructions; BACKOFF > 0 parks the warp that many nanoseconds between polls (roles with slack: their polls would
 // otherwise take issue slots from the working warps).
@@ -154,6 +155,7 @@ template <int BACKOFF> __device__ __forceinline__ void bf_wait_t(uint64_t *bar, 
 __device__ __forceinline__ void bf_wait(uint64_t *bar, uint32_t parity) { bf_wait_t<0>(bar, parity); }
 __device__ __forceinline__ void bf_wait_slack(uint64_t *bar, uint32_t parity) { bf_wait_t<0>(bar, parity); }
 
+// [ledger: a3 deconstruction: quantise, offset, byte planes]
 // append the 7 bytes of w = (hi:lo) (hi < 2^24) at byte position 7 e of a little-endian word array; e is a
 // compile-time constant after unrolling, so every index and shift folds
 __device__ __forceinline__ void bf_append7(uint32_t *wd, int e, uint32_t lo, uint32_t hi) {
@@ -166,6 +168,7 @@ __device__ __forceinline__ void bf_append7(uint32_t *wd, int e, uint32_t lo, uin
     }
 }
 
+// [ledger: setup, tile decode, loop control]
 template <int K>
 __global__ void __launch_bounds__(BF_THREADS, 1) stage_bf_kernel(StageGeom g, const uint4 *__restrict__ in, uint4 *__restrict__ out,
                                                                  const uint8_t *__restrict__ mat, const uint4 *__restrict__ ctab,
@@ -199,6 +202,7 @@ __global__ void __launch_bounds__(BF_THREADS, 1) stage_bf_kernel(StageGeom g, co
     const uint32_t tmem = s_tmem;
 
     if (warp == 0) {
+        // [ledger: a11 matrix stream (TMA bulk copies)]
         // ------------------------------------------------ matrix producer (whole warp walks the loop, one lane issues)
         uint32_t m = 0;
         for (long long tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
@@ -216,6 +220,7 @@ __global__ void __launch_bounds__(BF_THREADS, 1) stage_bf_kernel(StageGeom g, co
             }
         }
     } else if (warp == 1) {
+        // [ledger: a4 + a6 tensor-core issue (copies, stage MMAs, Phase-A MMAs)]
         // ------------------------------------------------ tensor-core issuer (one elected lane; program order = execution order)
         // per tile: tcgen05.cp of the data operand shared memory -> TMEM (then the shared copy is free for the next
         // tile); per chunk: a4 stage MMAs with A from TMEM (a3 and a5 folded into the operands), then a6 Phase A with
@@ -277,6 +282,7 @@ __global__ void __launch_bounds__(BF_THREADS, 1) stage_bf_kernel(StageGeom g, co
             }
         }
     } else if (warp >= 4 && warp < 12) {
+        // [ledger: a1 load + addressing]
         // ------------------------------------------------ deconstruction: thread = (column, parity of j)
         const int dw = warp - 4, par = lane >> 4, c = dw * 16 + (lane & 15);
         constexpr int BS = H < 8 ? H : 8;  // elements loaded together (memory-level parallelism)
@@ -289,6 +295,7 @@ __global__ void __launch_bounds__(BF_THREADS, 1) stage_bf_kernel(StageGeom g, co
             const bool valid = blk * 32 + (c & 31) < g.ncols;
             const uint4 *src = in + ((long long)blk * g.ib + (long long)ts * g.is + (long long)to * g.io + (long long)(c & 31) * g.lane + (long long)par * g.ji);
             const long long jstep = 2 * g.ji;
+            // [ledger: a2 column exponent]
             // a2: column exponent = max of the 11-bit exponent fields (integer compare on the high words)
             uint32_t hmax = 0;
 #pragma unroll
@@ -312,6 +319,7 @@ __global__ void __launch_bounds__(BF_THREADS, 1) stage_bf_kernel(StageGeom g, co
                 tm = max(tm, __shfl_xor_sync(0xFFFFFFFFu, tm, 16));
                 if (ef == 0 && tm > -100000) { flag = 1; Tmax = tm; }
             }
+            // [ledger: a3 deconstruction: quantise, offset, byte planes]
             // the previous tile's operand must have been copied to TMEM before the shared copy is overwritten
             if (it >= 1) bf_wait_slack(&a_empty[0], (it - 1) & 1);
             if (par == 0) { s_T[buf][c] = Tmax; s_flag[buf][c] = flag; }
@@ -361,6 +369,7 @@ __global__ void __launch_bounds__(BF_THREADS, 1) stage_bf_kernel(StageGeom g, co
             if (lane == 0) mbar_arrive(&a_full[0]);
         }
     } else if (warp >= 12) {
+        // [ledger: a12 store + addressing]
         // ------------------------------------------------ epilogue: thread = data column (TMEM lane), both parts
         const int qd = (warp - 12) >> 2, row = (warp & 3) * 32 + lane;
         const uint32_t lane_taddr = tmem + ((uint32_t)((warp & 3) * 32) << 16);
@@ -390,6 +399,7 @@ __global__ void __launch_bounds__(BF_THREADS, 1) stage_bf_kernel(StageGeom g, co
                     uint4 cc[2];
                     cc[0] = __ldg(ct + (kp < H ? kp : 0));
                     cc[1] = __ldg(ct + (kp < H ? kp + H : 0));
+                    // [ledger: a7 Phase B deposits (TMEM loads, slice sums -> E)]
                     bf_wait_slack(&pa_full[qd], nu & 1);
                     tc_fence_after();
                     uint32_t E[4][5];  // [part*2 + o]
@@ -405,6 +415,7 @@ __global__ void __launch_bounds__(BF_THREADS, 1) stage_bf_kernel(StageGeom g, co
                     if (lane == 0) mbar_arrive(&pa_empty[qd]);
                     nu++;
                     if (kp >= H || !valid) continue;
+                    // [ledger: a12 store + addressing]
                     uint4 *dk = dstp + (long long)kp * g.ko;
                     if (flag == 1) {  // the usual column: finite, not all zero
 #pragma unroll
@@ -428,6 +439,7 @@ __global__ void __launch_bounds__(BF_THREADS, 1) stage_bf_kernel(StageGeom g, co
                 }
         }
     }
+    // [ledger: setup, tile decode, loop control]
     tc_fence_before();
     __syncthreads();
     if (warp == 0) tmem_dealloc<512>(tmem);

@@ -11,11 +11,56 @@ namespace oz {
 constexpr int SIMT_THREADS = 256;
 constexpr int SIMT_KG = SIMT_THREADS / 32;
 
+// Reconstruction of one output from its 12 canonical residues.
+//   RECON 0: direct CRT with idempotents, fractional lift, two-sided centring -- the product form.
+//   RECON 1 (ablation): recursive Garner, Eq. (9)-(10) of PAPER.md:262-267: mixed-radix digits
+//            v_k = (v'_k - sum_{j<k} v_j prod_{i<j} m_i) (prod_{i<k} m_i)^-1 mod m_k, then the positional sum (Eq. 9).  Exact.
+//   RECON 2 (ablation): tc-CRT slice sums P_s followed by the NAIVE fp64 Phase B of PAPER.md:340-345 (Eq. 21):
+//            sum_s P_s c_s accumulated in fp64, rounding at every step.  The paper's naive form has no lift at all; to get a
+//            comparable output the quotient is taken in fp64 as well (rint(E/M)).  NOT exact: it is the accuracy-and-speed
+//            baseline, the only code in the library that uses fp64 arithmetic, excluded from the SASS hygiene test by name.
+template <int RECON> __device__ __forceinline__ uint64_t simt_reconstruct(const uint32_t *v, const DevConsts &c, int gexp) {
+    if constexpr (RECON == 0) {
+        return pack_rne(crt_centre(v, c), gexp);
+    } else if constexpr (RECON == 1) {
+        uint32_t d[12];
+#pragma unroll
+        for (int k = 0; k < 12; k++) {
+            const uint32_t m = c.m[k], mu = c.mu[k];
+            uint32_t acc = 0;  // sum_{j<k} d_j * gprod[j][k] mod m_k, one multiply-add-reduce per earlier digit (Eq. 10)
+#pragma unroll
+            for (int j = 0; j < k; j++) acc = barrett(acc + d[j] * (uint32_t)c.gprod[j][k], m, mu);
+            const uint32_t diff = v[k] >= acc ? v[k] - acc : v[k] + m - acc;
+            d[k] = barrett(diff * (uint32_t)c.ginv[k], m, mu);
+        }
+        u128 a = d[11];
+#pragma unroll
+        for (int k = 10; k >= 0; k--) a = a * c.m[k] + d[k];  // Eq. (9), Horner form
+        const u128 M = ((u128)c.M[3] << 96) | ((u128)c.M[2] << 64) | ((u128)c.M[1] << 32) | c.M[0];
+        i128 R = (i128)a;
+        if (a >= (M >> 1)) R -= (i128)M;
+        return pack_rne(R, gexp);
+    } else {
+        double e = 0.0;
+#pragma unroll
+        for (int s = 14; s >= 0; s--) {  // P_s = sum_k v_k byte_s(u_k) (Eq. 18-19), then sum_s P_s 256^s in fp64
+            uint32_t P = 0;
+#pragma unroll
+            for (int k = 0; k < 12; k++) P += v[k] * (uint32_t)c.uslice[k][s];
+            e = fma((double)P, exp2((double)(8 * s)), e);
+        }
+        const u128 M = ((u128)c.M[3] << 96) | ((u128)c.M[2] << 64) | ((u128)c.M[1] << 32) | c.M[0];
+        const double Md = (double)(uint64_t)(M >> 64) * 18446744073709551616.0 + (double)(uint64_t)M;
+        const double z = rint(e / Md);
+        const double r = fma(-z, Md, e);
+        return (uint64_t)__double_as_longlong(ldexp(r, -gexp));
+    }
+}
+
 // dynamic smem: bits[K][32] (16 B each) | xres[12][K][32] ushort2
-__global__ void __launch_bounds__(SIMT_THREADS) stage_simt_kernel(StageGeom g, const ulonglong2 *__restrict__ in,
-                                                                  ulonglong2 *__restrict__ out,
-                                                                  const ushort2 *__restrict__ mat,
-                                                                  const DevConsts *__restrict__ cptr) {
+template <int RECON>
+__device__ __forceinline__ void stage_simt_body(const StageGeom &g, const ulonglong2 *__restrict__ in, ulonglong2 *__restrict__ out,
+                                                const ushort2 *__restrict__ mat, const DevConsts *__restrict__ cptr) {
     extern __shared__ __align__(16) uint8_t smem_raw[];
     __shared__ int s_tmax[32];
     __shared__ int s_flag[32];  // bit0: some nonzero finite, bit1: non-finite
@@ -91,11 +136,24 @@ __global__ void __launch_bounds__(SIMT_THREADS) stage_simt_kernel(StageGeom g, c
                 vr[i] = barrett((uint32_t)(re + (int)c.off28[i]), c.m[i], c.mu[i]);
                 vi[i] = barrett((uint32_t)(im + (int)c.off28[i]), c.m[i], c.mu[i]);
             }
-            y.x = pack_rne(crt_centre(vr, c), gexp);
-            y.y = pack_rne(crt_centre(vi, c), gexp);
+            y.x = simt_reconstruct<RECON>(vr, c, gexp);
+            y.y = simt_reconstruct<RECON>(vi, c, gexp);
         }
         if (valid) out[obase + k * g.ko] = y;
     }
+}
+
+__global__ void __launch_bounds__(SIMT_THREADS) stage_simt_kernel(StageGeom g, const ulonglong2 *__restrict__ in, ulonglong2 *__restrict__ out,
+                                                                  const ushort2 *__restrict__ mat, const DevConsts *__restrict__ cptr) {
+    stage_simt_body<0>(g, in, out, mat, cptr);
+}
+__global__ void __launch_bounds__(SIMT_THREADS) stage_garner_kernel(StageGeom g, const ulonglong2 *__restrict__ in, ulonglong2 *__restrict__ out,
+                                                                    const ushort2 *__restrict__ mat, const DevConsts *__restrict__ cptr) {
+    stage_simt_body<1>(g, in, out, mat, cptr);
+}
+__global__ void __launch_bounds__(SIMT_THREADS) stage_fp64sum_kernel(StageGeom g, const ulonglong2 *__restrict__ in, ulonglong2 *__restrict__ out,
+                                                                     const ushort2 *__restrict__ mat, const DevConsts *__restrict__ cptr) {
+    stage_simt_body<2>(g, in, out, mat, cptr);
 }
 
 }  // namespace oz

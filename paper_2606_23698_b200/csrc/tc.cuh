@@ -6,6 +6,8 @@
 
 namespace oz {
 
+// [ledger: sync: mbarrier waits]
+
 // ---- instruction descriptor (32 bit, passed as the 4th mma operand) ----
 enum : uint32_t { CFMT_F16 = 0, CFMT_F32 = 1, CFMT_S32 = 2 };
 enum : uint32_t { F8_E4M3 = 0, F8_E5M2 = 1, F16_F16 = 0, F16_BF16 = 1, I8_U8 = 0, I8_S8 = 1 };
