@@ -254,6 +254,15 @@ bool add_axis(ozfft_plan_s *p, const AxisDesc &a, int axis, MatMap &mats, std::v
         g2.lane = a.N; g2.ji = 1; g2.ko = 32; g2.order = 1;
     }
     g1.ob = g1.ib; g1.os = g1.is; g1.oo = g1.io;
+    g1.olane = g1.lane; g2.olane = g2.lane;
+    if (a.contiguous && two && pp == 32) {
+        // N = 1024 on the contiguous axis: the array between the two stages is ours to lay out.  Y'[k2][pencil][j1]
+        // (instead of the input's own positions) makes a second-stage tile -- 128 pencils that share k2 -- one
+        // contiguous 64 KB read; the first stage still writes 512-byte runs (32 lanes along j1).
+        const long long Pn = a.outer;
+        g1.ob = 32; g1.ko = Pn * 32;
+        g2.ib = 32 * 32; g2.lane = 32; g2.ji = 1; g2.is = Pn * 32;
+    }
     if (!get(q, 0, s1)) return false;
     dst.push_back(s1);
     if (two) {

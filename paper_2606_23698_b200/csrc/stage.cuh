@@ -16,7 +16,8 @@ struct StageGeom {
     int ncols;           // columns along the b coordinate: column 32 b + lane exists iff it is < ncols (masked tail block)
     long long ib, is, io;  // input base strides per block coordinate
     long long ob, os, oo;  // output base strides
-    long long lane;      // stride between the 32 columns of a block (same for input and output)
+    long long lane;      // stride between the 32 columns of a block in the input
+    long long olane;     // the same in the output
     long long ji;        // input stride between contraction elements j
     long long ko;        // output stride between output rows k
     int matsel;          // matrix index of a block: 0 -> 0, 1 -> s

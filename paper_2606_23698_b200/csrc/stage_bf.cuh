@@ -156,6 +156,11 @@ __device__ __forceinline__ void bf_wait(uint64_t *bar, uint32_t parity) { bf_wai
 __device__ __forceinline__ void bf_wait_slack(uint64_t *bar, uint32_t parity) { bf_wait_t<0>(bar, parity); }
 
 // [ledger: a3 deconstruction: quantise, offset, byte planes]
+// tile of iteration `it` of this CTA: CTAs take PAIRS of consecutive tiles.  In the second stage of the contiguous axis
+// consecutive tiles are k2, k2+1 over the same pencils, whose 16-byte outputs are the two halves of the same 32-byte
+// sectors: written by one SM back to back they merge in L2 instead of reaching DRAM as partial (read-modify-write) sectors.
+__device__ __forceinline__ long long bf_tile(long long it) { return ((it >> 1) * gridDim.x + blockIdx.x) * 2 + (it & 1); }
+
 // append the 7 bytes of w = (hi:lo) (hi < 2^24) at byte position 7 e of a little-endian word array; e is a
 // compile-time constant after unrolling, so every index and shift folds
 __device__ __forceinline__ void bf_append7(uint32_t *wd, int e, uint32_t lo, uint32_t hi) {
@@ -205,7 +210,7 @@ __global__ void __launch_bounds__(BF_THREADS, 1) stage_bf_kernel(StageGeom g, co
         // [ledger: a11 matrix stream (TMA bulk copies)]
         // ------------------------------------------------ matrix producer (whole warp walks the loop, one lane issues)
         uint32_t m = 0;
-        for (long long tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
+        for (long long pit = 0, tile; (tile = bf_tile(pit)) < ntiles; pit++) {
             int tb, ts, to;
             tile_coords_pow2(g, tile, lg_nbt, lg_ns, tb, ts, to);
             const uint8_t *mb = mat + (size_t)(g.matsel ? ts : 0) * bf_mat_bytes(K);
@@ -230,7 +235,7 @@ __global__ void __launch_bounds__(BF_THREADS, 1) stage_bf_kernel(StageGeom g, co
         const uint64_t adesc0 = make_sdesc(smem_u32(sA), BF_COLS * 16, 128);
         constexpr int ACOLS = 3 * NCK * 4;  // TMEM columns of one parity of the data operand
         uint32_t m = 0, n = 0, it = 0;
-        for (long long tile = blockIdx.x; tile < ntiles; tile += gridDim.x, it++) {
+        for (long long tile; (tile = bf_tile(it)) < ntiles; it++) {
             bf_wait(&a_full[0], it & 1);
             tc_fence_after();
             if (elect_one()) {
@@ -287,7 +292,7 @@ __global__ void __launch_bounds__(BF_THREADS, 1) stage_bf_kernel(StageGeom g, co
         const int dw = warp - 4, par = lane >> 4, c = dw * 16 + (lane & 15);
         constexpr int BS = H < 8 ? H : 8;  // elements loaded together (memory-level parallelism)
         uint32_t it = 0;
-        for (long long tile = blockIdx.x; tile < ntiles; tile += gridDim.x, it++) {
+        for (long long tile; (tile = bf_tile(it)) < ntiles; it++) {
             const uint32_t buf = it & 1;
             int tb, ts, to;
             tile_coords_pow2(g, tile, lg_nbt, lg_ns, tb, ts, to);
@@ -375,13 +380,13 @@ __global__ void __launch_bounds__(BF_THREADS, 1) stage_bf_kernel(StageGeom g, co
         const uint32_t lane_taddr = tmem + ((uint32_t)((warp & 3) * 32) << 16);
         uint32_t it = 0, nu = 0;  // tiles seen, units this group has consumed
         int turn = qd;            // units to skip until the next one of this group (units go round-robin over the 3 groups)
-        for (long long tile = blockIdx.x; tile < ntiles; tile += gridDim.x, it++) {
+        for (long long tile; (tile = bf_tile(it)) < ntiles; it++) {
             const uint32_t buf = it & 1;
             int tb, ts, to;
             tile_coords_pow2(g, tile, lg_nbt, lg_ns, tb, ts, to);
             const int blk = 4 * tb + (row >> 5);
             const bool valid = blk * 32 + (row & 31) < g.ncols;
-            uint4 *dstp = out + ((long long)blk * g.ob + (long long)ts * g.os + (long long)to * g.oo + (long long)(row & 31) * g.lane);
+            uint4 *dstp = out + ((long long)blk * g.ob + (long long)ts * g.os + (long long)to * g.oo + (long long)(row & 31) * g.olane);
             const uint4 *ct = ctab + (size_t)(g.matsel ? ts : 0) * K;
             bf_wait_slack(&a_full[0], it & 1);  // the column exponents of this tile are published (s_T is double buffered: the
             const int Tmax = s_T[buf][row], flag = s_flag[buf][row];  // deconstruction runs at most one tile ahead)
@@ -448,7 +453,8 @@ __global__ void __launch_bounds__(BF_THREADS, 1) stage_bf_kernel(StageGeom g, co
 template <int K>
 inline bool stage_bf_launch_k(const StageGeom &g, const void *in, void *out, const uint8_t *mat, const void *ctab, const void *pa,
                               long long nt, int sms, cudaStream_t st) {
-    const unsigned grid = (unsigned)(nt < sms ? nt : sms);
+    const long long pairs = (nt + 1) / 2;  // CTAs walk pairs of consecutive tiles (bf_tile)
+    const unsigned grid = (unsigned)(pairs < sms ? pairs : sms);
     stage_bf_kernel<K><<<grid, BF_THREADS, bf_smem_bytes<K>(), st>>>(g, (const uint4 *)in, (uint4 *)out, mat, (const uint4 *)ctab, (const uint4 *)pa, nt);
     return cudaGetLastError() == cudaSuccess;
 }

@@ -77,7 +77,7 @@ __device__ __forceinline__ void stage_simt_body(const StageGeom &g, const ulongl
     int tb, ts, to;
     tile_coords(g, blockIdx.x, g.nb, tb, ts, to);
     const long long ibase = tb * g.ib + ts * g.is + to * g.io + lane * g.lane;
-    const long long obase = tb * g.ob + ts * g.os + to * g.oo + lane * g.lane;
+    const long long obase = tb * g.ob + ts * g.os + to * g.oo + lane * g.olane;
     const int mid = g.matsel ? ts : 0;
     const bool valid = tb * 32 + lane < g.ncols;  // masked tail block
 

@@ -116,7 +116,7 @@ __global__ void __launch_bounds__(128 * tc_q(KP), KP >= 32 ? 1 : 2) stage_tc_ker
         const int blk = 2 * tb + (col >> 5);
         valid = blk * 32 + (col & 31) < g.ncols;
         ib = (uint32_t)blk * (uint32_t)g.ib + (uint32_t)ts * (uint32_t)g.is + (uint32_t)to * (uint32_t)g.io + (uint32_t)(col & 31) * (uint32_t)g.lane;
-        ob = (uint32_t)blk * (uint32_t)g.ob + (uint32_t)ts * (uint32_t)g.os + (uint32_t)to * (uint32_t)g.oo + (uint32_t)(col & 31) * (uint32_t)g.lane;
+        ob = (uint32_t)blk * (uint32_t)g.ob + (uint32_t)ts * (uint32_t)g.os + (uint32_t)to * (uint32_t)g.oo + (uint32_t)(col & 31) * (uint32_t)g.olane;
         mb = mat + (size_t)(g.matsel ? ts : 0) * 12 * MB;
     };
     const uint32_t ji32 = (uint32_t)g.ji, ko32 = (uint32_t)g.ko;
