@@ -16,6 +16,7 @@
 #include "stage_simt.cuh"
 #include "stage_tc.cuh"
 #include "stage_bf.cuh"
+#include "stage_f8.cuh"
 #include "tables.cuh"
 #include "probe.cuh"
 
@@ -47,6 +48,7 @@ struct StageLaunch {
     const ushort2 *mat_simt;  // [nmat][12][K][K] (a_R, a_I) canonical residues
     const uint8_t *mat_tc;    // digit planes for the tensor-core kernel (stage_tc.cuh)
     const uint8_t *mat_bf;    // matrix byte planes of the byte-fed kernel (stage_bf.cuh)
+    const uint8_t *mat_f8;    // E4M3 hex-digit planes of the FP8 rung (stage_f8.cuh)
     const void *ctab_bf;      // its offset constants [nmat][K] x 16 B
     int axis;
 };
@@ -57,7 +59,7 @@ struct ozfft_plan_s {
     uint32_t magic;
     int nx, ny, nz, sign;
     long long count;
-    int variant;  // 0 simt, 1 tensor-core (residue digits), 2 byte-fed tensor-core (default), 3 / 4 ablations on the simt kernel
+    int variant;  // 0 simt, 1 tensor-core (residue digits), 2 byte-fed tensor-core (default), 3 / 4 ablations on the simt kernel, 5 FP8 rung
     int sms;      // SM count of the plan's device
     int tc_per_sm[3];  // resident CTAs per SM of the residue-digit kernel instantiations (per device)
     const void *pa_bf;  // Phase-A constant matrix of the byte-fed kernel
@@ -156,7 +158,7 @@ struct MatKey {
 };
 struct MatSet {
     const ushort2 *simt;
-    const uint8_t *tc, *bf;
+    const uint8_t *tc, *bf, *f8;
     const void *ctab;
 };
 typedef std::map<MatKey, MatSet> MatMap;
@@ -201,7 +203,7 @@ bool add_axis(ozfft_plan_s *p, const AxisDesc &a, int axis, MatMap &mats, std::v
         auto it = mats.find(key);
         if (it == mats.end()) {
             MatSet ms{};
-            if (p->variant == 0 || p->variant >= 3) {
+            if (p->variant == 0 || p->variant == 3 || p->variant == 4) {
                 ms.simt = build_mat_simt(p, K, fusedN);
                 if (!ms.simt) return false;
             } else if (p->variant == 1) {
@@ -209,6 +211,11 @@ bool add_axis(ozfft_plan_s *p, const AxisDesc &a, int axis, MatMap &mats, std::v
                 build_mat_tc(h, K, fusedN, p->sign, twiddles());
                 ms.tc = (const uint8_t *)dev_upload(p, h.data(), h.size());
                 if (!ms.tc) return false;
+            } else if (p->variant == 5) {
+                std::vector<uint8_t> h;
+                build_mat_f8(h, K, fusedN, p->sign, twiddles());
+                ms.f8 = (const uint8_t *)dev_upload(p, h.data(), h.size());
+                if (!ms.f8) return false;
             } else {
                 std::vector<uint8_t> h;
                 std::vector<uint32_t> c;
@@ -222,6 +229,7 @@ bool add_axis(ozfft_plan_s *p, const AxisDesc &a, int axis, MatMap &mats, std::v
         s.mat_simt = it->second.simt;
         s.mat_tc = it->second.tc;
         s.mat_bf = it->second.bf;
+        s.mat_f8 = it->second.f8;
         s.ctab_bf = it->second.ctab;
         return true;
     };
@@ -277,7 +285,8 @@ int pick_variant() {
     if (v && !strcmp(v, "simt")) return 0;
     if (v && !strcmp(v, "tc")) return 1;
     if (v && !strcmp(v, "garner")) return 3;   // ablation: SIMT kernel with recursive Garner reconstruction
-    if (v && !strcmp(v, "fp64sum")) return 4;  // ablation: SIMT kernel with the naive fp64 Phase B (NOT exact, uses fp64)
+    if (v && !strcmp(v, "fp64sum")) return 4;
+    if (v && !strcmp(v, "fp8")) return 5;      // measured rung: kind::f8f6f4 E4M3 digit planes + residue-domain Karatsuba  // ablation: SIMT kernel with the naive fp64 Phase B (NOT exact, uses fp64)
     return 2;
 }
 
@@ -332,13 +341,14 @@ ozfft_plan_s *make_plan(int nx, int ny, int nz, int sign, bool batched1d) {
         if (ok) p->dev_bytes += (size_t)p->count * 16;
     }
     // per plan, on the plan's device: kernel attributes and the constant bank (both are per-device state)
-    if (ok && (p->variant == 0 || p->variant >= 3)) {
+    if (ok && (p->variant == 0 || p->variant == 3 || p->variant == 4)) {
         const int sm = 32 * 32 * 16 + 12 * 32 * 32 * 4;
         ok = cuda_ok(cudaFuncSetAttribute(stage_simt_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, sm), "cudaFuncSetAttribute") &&
              cuda_ok(cudaFuncSetAttribute(stage_garner_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, sm), "cudaFuncSetAttribute") &&
              cuda_ok(cudaFuncSetAttribute(stage_fp64sum_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, sm), "cudaFuncSetAttribute");
     }
-    if (ok && (p->variant == 1 || p->variant == 2)) ok = stage_tc_prepare(hc);  // uploads the constant bank both tensor-core kernels read
+    if (ok && (p->variant == 1 || p->variant == 2 || p->variant == 5)) ok = stage_tc_prepare(hc);
+    if (ok && p->variant == 5) ok = stage_f8_prepare();  // uploads the constant bank both tensor-core kernels read
     if (ok && p->variant == 1) stage_tc_occupancy(p->tc_per_sm);
     if (ok && p->variant == 2) ok = stage_bf_prepare();
     if (!ok && g_err.empty()) set_err("kernel attribute setup failed");
@@ -362,6 +372,9 @@ bool valid(ozfft_plan p) {
 
 int launch_stage(ozfft_plan p, const StageLaunch &s, const void *src, void *dst, cudaStream_t st) {
     const long long nt = (long long)s.g.nb * s.g.ns * s.g.no;
+    if (p->variant == 5) {
+        return cuda_ok(stage_f8_launch(s.g, src, dst, s.mat_f8, p->sms, st), "stage_f8_kernel launch") ? OZFFT_OK : OZFFT_ECUDA;
+    }
     if (p->variant == 2) {
         if (stage_bf_launch(s.g, src, dst, s.mat_bf, s.ctab_bf, p->pa_bf, p->sms, st)) return OZFFT_OK;
         set_err(std::string("stage_bf_kernel launch: ") + cudaGetErrorString(cudaGetLastError()));

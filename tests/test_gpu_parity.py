@@ -8,10 +8,10 @@ pytestmark = pytest.mark.gpu
 TOL_F128 = 5e-15  # north_star: normwise relative error vs the __float128 naive DFT
 
 
-@pytest.fixture(autouse=True, params=["bf", "tc", "simt"])
+@pytest.fixture(autouse=True, params=["bf", "tc", "simt", "fp8"])
 def variant(request, monkeypatch):
     """every parity case runs on the byte-fed tensor-core kernel (the default), on the residue-digit tensor-core
-    kernel and on the all-SIMT cross-check kernel"""
+    kernel, on the all-SIMT cross-check kernel and on the FP8 (kind::f8f6f4 + Karatsuba) rung"""
     monkeypatch.setenv("OZFFT_VARIANT", request.param)
     return request.param
 

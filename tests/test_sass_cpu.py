@@ -56,6 +56,8 @@ def test_tensor_core_kernels_are_blackwell_native():
     for k, v in ks.items():
         if "stage_tc_kernel" in k:
             ops = ("UTCIMMA", "LDTM", "UBLKCP", "SYNCS")
+        elif "stage_f8_kernel" in k:
+            ops = ("UTCQMMA", "LDTM", "UBLKCP", "SYNCS")  # kind::f8f6f4 -> UTCQMMA
         elif "stage_bf_kernel" in k:
             ops = ("UTCIMMA", "UTCCP", "LDTM", "UBLKCP", "SYNCS", "ELECT", "LDG.E.128", "STG.E.128")
         else:
@@ -63,3 +65,4 @@ def test_tensor_core_kernels_are_blackwell_native():
         for op in ops:
             assert op in v, (k, op)
         assert "HMMA" not in v and "IMMA." not in v.replace("UTCIMMA", "")
+    assert any("stage_f8_kernel" in k for k in ks)
