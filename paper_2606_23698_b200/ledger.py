@@ -16,7 +16,7 @@ markers of the file they are defined in), and prints
   * c_q^res: deconstruction thread instructions per element and modulus (PAPER.md:190, 441: 3.0 - 6.3);
   * the issue ceiling these counts imply at 148 SM x 128 lanes x 1.965 GHz.
 
-Nothing here runs on the GPU and nothing is imported from oracle/.
+Nothing here runs on the GPU and no module under oracle/ is used.
 """
 import argparse
 import collections
