@@ -64,6 +64,7 @@ struct ozfft_plan_s {
     int tc_per_sm[3];  // resident CTAs per SM of the residue-digit kernel instantiations (per device)
     const void *pa_bf;  // Phase-A constant matrix of the byte-fed kernel
     std::vector<StageLaunch> stages;
+    std::vector<StageLaunch> stages_nat;  // the same passes with every intermediate array in natural order (ozfft_exec_axis)
     std::vector<void *> dev_allocs;
     size_t dev_bytes;
     DevConsts *d_consts;
@@ -194,7 +195,9 @@ struct AxisDesc {
     long long outer, N, inner;  // strided: element (o, i, z) at (o*N + i)*inner + z; contiguous: pencil P at P*N
 };
 
-bool add_axis(ozfft_plan_s *p, const AxisDesc &a, int axis, MatMap &mats, std::vector<StageLaunch> &dst) {
+// perm_out: the second stage of this (contiguous) axis writes index k1 + p k2 instead of k2 + 32 k1; unperm = p > 0: the first
+// stage of this axis reads an inner index permuted that way and writes the natural one (StageGeom::patch)
+bool add_axis(ozfft_plan_s *p, const AxisDesc &a, int axis, MatMap &mats, std::vector<StageLaunch> &dst, bool perm_out = false, int unperm = 0) {
     const int N = (int)a.N;
     const bool two = N > 32;
     const int q = two ? 32 : N, pp = two ? N / 32 : 1;
@@ -271,6 +274,15 @@ bool add_axis(ozfft_plan_s *p, const AxisDesc &a, int axis, MatMap &mats, std::v
         g1.ob = 32; g1.ko = Pn * 32;
         g2.ib = 32 * 32; g2.lane = 32; g2.ji = 1; g2.is = Pn * 32;
     }
+    if (perm_out) { g2.os = pp; g2.ko = 1; }
+    for (StageGeom *gp : {&g1, &g2}) {  // column addressing of the byte-fed kernel: four blocks of 32 lanes
+        gp->ci = StageGeom::ColMap{0, 0, 31, 5, 4 * gp->ib, 0, gp->lane, gp->ib};
+        gp->co = StageGeom::ColMap{0, 0, 31, 5, 4 * gp->ob, 0, gp->olane, gp->ob};
+    }
+    if (unperm) {  // 8 (k1) x 16 (k2) patch: permuted index k1 + p k2 in, natural index k2 + 32 k1 out
+        g1.ci = StageGeom::ColMap{1, 1, 7, 3, 8, 16LL * unperm, 1, unperm};
+        g1.co = StageGeom::ColMap{1, 1, 7, 3, 256, 16, 32, 1};
+    }
     if (!get(q, 0, s1)) return false;
     dst.push_back(s1);
     if (two) {
@@ -324,15 +336,22 @@ ozfft_plan_s *make_plan(int nx, int ny, int nz, int sign, bool batched1d) {
     if (batched1d) {  // nx = batch, nz = n
         ok = ok && add_axis(p, AxisDesc{true, nx, nz, 1}, 0, mats, p->stages);
     } else {
-        ok = ok && add_axis(p, AxisDesc{true, (long long)nx * ny, nz, 1}, 0, mats, p->stages);
-        ok = ok && add_axis(p, AxisDesc{false, nx, ny, nz}, 1, mats, p->stages);
+        // byte-fed kernel, nz >= 256: the z pass leaves its output permuted along z and the first y stage undoes it (stage.cuh)
+        const bool perm = p->variant == 2 && nz >= 256;
+        ok = ok && add_axis(p, AxisDesc{true, (long long)nx * ny, nz, 1}, 0, mats, p->stages, perm, 0);
+        ok = ok && add_axis(p, AxisDesc{false, nx, ny, nz}, 1, mats, p->stages, false, perm ? nz / 32 : 0);
         ok = ok && add_axis(p, AxisDesc{false, 1, nx, (long long)ny * nz}, 2, mats, p->stages);
+        if (perm) {
+            ok = ok && add_axis(p, AxisDesc{true, (long long)nx * ny, nz, 1}, 0, mats, p->stages_nat);
+            ok = ok && add_axis(p, AxisDesc{false, nx, ny, nz}, 1, mats, p->stages_nat);
+            ok = ok && add_axis(p, AxisDesc{false, 1, nx, (long long)ny * nz}, 2, mats, p->stages_nat);
+        }
         // host-buffer pipeline (ozfft_exec_host): the z and y passes run per slab of nx/8 planes as the slabs arrive,
         // the x pass per chunk of ny/8 rows whose results leave while the next chunk computes
         const int xs = nx / PIPE, yc = ny / PIPE;
         if (ok && nx >= PIPE && ny >= PIPE && p->count >= (1ll << 24) && ((long long)xs * ny) % 64 == 0 && ((long long)yc * nz) % 64 == 0) {
-            ok = ok && add_axis(p, AxisDesc{true, (long long)xs * ny, nz, 1}, 0, mats, p->slab_stages);
-            ok = ok && add_axis(p, AxisDesc{false, xs, ny, nz}, 1, mats, p->slab_stages);
+            ok = ok && add_axis(p, AxisDesc{true, (long long)xs * ny, nz, 1}, 0, mats, p->slab_stages, perm, 0);
+            ok = ok && add_axis(p, AxisDesc{false, xs, ny, nz}, 1, mats, p->slab_stages, false, perm ? nz / 32 : 0);
             p->pipelined = ok;
         }
     }
@@ -393,12 +412,12 @@ int launch_stage(ozfft_plan p, const StageLaunch &s, const void *src, void *dst,
 }
 
 // run stages [first, last) : src -> ... -> dst, alternating through the plan workspace so the last lands in dst
-int run_stages(ozfft_plan p, size_t first, size_t last, const void *in, void *out, cudaStream_t st) {
+int run_stages(ozfft_plan p, const std::vector<StageLaunch> &stages, size_t first, size_t last, const void *in, void *out, cudaStream_t st) {
     const size_t L = last - first;
     const void *src = in;
     for (size_t i = 0; i < L; i++) {
         void *dst = ((L - 1 - i) & 1) ? p->work : out;
-        int rc = launch_stage(p, p->stages[first + i], src, dst, st);
+        int rc = launch_stage(p, stages[first + i], src, dst, st);
         if (rc) return rc;
         src = dst;
     }
@@ -436,17 +455,18 @@ ozfft_plan ozfft_plan_create_1d(int n, int batch, int sign) {
 int ozfft_exec(ozfft_plan p, const void *in, void *out, void *stream) {
     if (!valid(p)) { set_err("invalid or destroyed plan"); return OZFFT_EINVAL; }
     if (!check_ptrs(in, out)) return OZFFT_EINVAL;
-    return run_stages(p, 0, p->stages.size(), in, out, (cudaStream_t)stream);
+    return run_stages(p, p->stages, 0, p->stages.size(), in, out, (cudaStream_t)stream);
 }
 
 int ozfft_exec_axis(ozfft_plan p, int axis, const void *in, void *out, void *stream) {
     if (!valid(p)) { set_err("invalid or destroyed plan"); return OZFFT_EINVAL; }
     if (!check_ptrs(in, out)) return OZFFT_EINVAL;
-    size_t first = p->stages.size(), last = 0;
-    for (size_t i = 0; i < p->stages.size(); i++)
-        if (p->stages[i].axis == axis) { first = i < first ? i : first; last = i + 1; }
+    const std::vector<StageLaunch> &sl = p->stages_nat.empty() ? p->stages : p->stages_nat;  // natural order in, natural order out
+    size_t first = sl.size(), last = 0;
+    for (size_t i = 0; i < sl.size(); i++)
+        if (sl[i].axis == axis) { first = i < first ? i : first; last = i + 1; }
     if (first >= last) { set_err("no such axis in this plan"); return OZFFT_EINVAL; }
-    return run_stages(p, first, last, in, out, (cudaStream_t)stream);
+    return run_stages(p, sl, first, last, in, out, (cudaStream_t)stream);
 }
 
 // pipelined host-buffer transform of a 3-D plan: H2D slab s || z,y passes of slab s-1;  x pass of chunk c || D2H of chunk c-1
@@ -528,7 +548,7 @@ int ozfft_exec_host(ozfft_plan p, const void *host_in, void *host_out, void *str
     cudaStream_t st = (cudaStream_t)stream;
     if (p->pipelined && !getenv("OZFFT_NO_PIPELINE")) return exec_host_pipelined(p, (const char *)host_in, (char *)host_out, st);
     if (!cuda_ok(cudaMemcpyAsync(p->h_in, host_in, bytes, cudaMemcpyHostToDevice, st), "H2D")) return OZFFT_ECUDA;
-    int rc = run_stages(p, 0, p->stages.size(), p->h_in, p->h_out, st);
+    int rc = run_stages(p, p->stages, 0, p->stages.size(), p->h_in, p->h_out, st);
     if (rc) return rc;
     if (!cuda_ok(cudaMemcpyAsync(host_out, p->h_out, bytes, cudaMemcpyDeviceToHost, st), "D2H")) return OZFFT_ECUDA;
     return cuda_ok(cudaStreamSynchronize(st), "cudaStreamSynchronize") ? OZFFT_OK : OZFFT_ECUDA;
@@ -584,6 +604,10 @@ size_t ozfft_debug_bf_tables(int K, int fusedN, int sign, void *h_B, void *h_C, 
     }
     return B.size();
 }
+
+#ifdef OZFFT_PIPE_TIMERS
+void ozfft_debug_timers(unsigned long long *h) { cudaMemcpyFromSymbol(h, g_bf_dbg, sizeof(g_bf_dbg)); }
+#endif
 
 uint64_t ozfft_twiddle_checksum(void) { return twiddle_fnv(twiddles()); }
 

@@ -25,6 +25,7 @@
 //
 // Capacity: |R + C| <= 2^111.5 + 2^111.5 < M/2 = 2^116.9.  E < 30768 M < 2^134.
 #pragma once
+#include <utility>
 #include <vector>
 
 #include "arith.cuh"
@@ -129,8 +130,10 @@ inline void build_pa_bf(uint8_t *pa, const CrtConsts &C) {
 // warp 2 = Phase-A MMA issuer, warp 3 idle, warps 4-11 = deconstruction (a1-a3: load, column exponent, quantise, byte planes),
 // warps 12-23 = epilogue (a7-a9, a12: deposits, lift, pack, store; three groups of four warps, one TMEM lane
 // quarter each).  All hand-offs are mbarriers; there is no block-wide barrier inside the tile loop.
-constexpr int BF_THREADS = 768;
-constexpr int BF_NSLOT = 12;        // matrix ring slots (one parity of one chunk each)
+constexpr int BF_NG = 3;            // epilogue groups of four warps (units go round-robin over them)
+constexpr int BF_THREADS = 128 * (3 + BF_NG);
+constexpr int BF_NSLOT = 8;         // matrix ring: half-slots of one parity of one chunk; a ring entry is one chunk (two of them)
+constexpr int BF_NCS = BF_NSLOT / 2;
 // TMEM columns: [0,168) data operand (per parity 84: XI | XR | NXI, 4 columns per 16-byte chunk), [168,360) stage
 // accumulators of one chunk ([re rows: E 48 | O 48][im rows: E 48 | O 48]), [360,488) Phase-A results (2 slots x 64)
 constexpr int BF_TA = 0, BF_TD = 168, BF_DPA = 360;
@@ -138,6 +141,14 @@ template <int K> __host__ __device__ constexpr size_t bf_smem_bytes() {
     return (size_t)bf_aset_bytes(K) + (size_t)BF_NSLOT * bf_slot_bytes(K) + BF_PA_BYTES;
 }
 
+#ifdef OZFFT_PIPE_TIMERS
+__device__ unsigned long long g_bf_dbg[160][8];
+#define OZ_T0() const long long t0_ = clock64()
+#define OZ_T1(i) dbg_[i] += clock64() - t0_
+#else
+#define OZ_T0()
+#define OZ_T1(i)
+#endif
 // [ledger: sync: mbarrier waits]
 // bounded wait: a pipeline bug must not hang the GPU (traps after 2^26 failed polls).  The poll loop is four
 // instructions; BACKOFF > 0 parks the warp that many nanoseconds between polls (roles with slack: their polls would
@@ -153,6 +164,7 @@ template <int BACKOFF> __device__ __forceinline__ void bf_wait_t(uint64_t *bar, 
     } while (!done);
 }
 __device__ __forceinline__ void bf_wait(uint64_t *bar, uint32_t parity) { bf_wait_t<0>(bar, parity); }
+__device__ __forceinline__ void bf_wait_pa(uint64_t *bar, uint32_t parity) { bf_wait_t<0>(bar, parity); }
 __device__ __forceinline__ void bf_wait_slack(uint64_t *bar, uint32_t parity) { bf_wait_t<0>(bar, parity); }
 
 // [ledger: a3 deconstruction: quantise, offset, byte planes]
@@ -182,7 +194,7 @@ __global__ void __launch_bounds__(BF_THREADS, 1) stage_bf_kernel(StageGeom g, co
     constexpr int SB = bf_slot_bytes(K), PLANE = bf_plane_bytes(K), ASET = bf_aset_bytes(K), PARB = NCK * BF_COLS * 16;
     constexpr int NW = PB / 4;
     extern __shared__ __align__(128) uint8_t smem[];
-    __shared__ __align__(8) uint64_t a_full[1], a_empty[1], e_start[1], b_full[BF_NSLOT], b_empty[BF_NSLOT], pa_full[3], pa_empty[3];
+    __shared__ __align__(8) uint64_t a_full[1], a_empty[1], e_start[1], b_full[BF_NCS], b_empty[BF_NCS], pa_full[BF_NG], pa_empty[1];
     __shared__ uint32_t s_tmem;
     __shared__ int s_T[2][BF_COLS], s_flag[2][BF_COLS];
     uint8_t *sA = smem, *sB = smem + ASET, *sPA = sB + BF_NSLOT * SB;
@@ -193,11 +205,13 @@ __global__ void __launch_bounds__(BF_THREADS, 1) stage_bf_kernel(StageGeom g, co
     for (int i = tid; i < BF_PA_BYTES / 16; i += BF_THREADS) ((uint4 *)sPA)[i] = __ldg(pa_g + i);
     if (warp == 0) tmem_alloc<512>(&s_tmem);
     if (tid == 0) {
-        // pa_full / pa_empty are per epilogue group (a waiter must see every phase of its barrier in turn:
+        // pa_full is per epilogue group; pa_empty counts the eight warps that drain the two units of one chunk (the two D_PA
+        // slots hold exactly one chunk; a waiter must see every phase of its barrier in turn:
         // try_wait on parity p passes at once while the barrier is still in the phase before p)
-        mbar_init(&a_full[0], 8); mbar_init(&a_empty[0], 1); mbar_init(&e_start[0], 12);
-        for (int i = 0; i < 3; i++) { mbar_init(&pa_full[i], 1); mbar_init(&pa_empty[i], 4); }
-        for (int i = 0; i < BF_NSLOT; i++) { mbar_init(&b_full[i], 1); mbar_init(&b_empty[i], 1); }
+        mbar_init(&a_full[0], 8); mbar_init(&a_empty[0], 1); mbar_init(&e_start[0], 4 * BF_NG);
+        for (int i = 0; i < BF_NG; i++) mbar_init(&pa_full[i], 1);
+        mbar_init(&pa_empty[0], 8);
+        for (int i = 0; i < BF_NCS; i++) { mbar_init(&b_full[i], 1); mbar_init(&b_empty[i], 1); }
         mbar_fence_init();
     }
     fence_async_smem();
@@ -205,21 +219,28 @@ __global__ void __launch_bounds__(BF_THREADS, 1) stage_bf_kernel(StageGeom g, co
     __syncthreads();
     tc_fence_after();
     const uint32_t tmem = s_tmem;
+    if (tmem != 0) __trap();  // the CTA owns all 512 columns of its SM: the allocation starts at lane 0, column 0
 
+    // register budget per role (setmaxnreg, per warpgroup): control 32, deconstruction 80, epilogue 64 (the launch value)
+    // slot uses of the matrix ring per tile and per slot: with an even number of uses per slot and tile (K = 32) every
+    // ring index and barrier parity below is a compile-time constant after unrolling
+    constexpr int UPT = (NCH + BF_NCS - 1) / BF_NCS;
+    static_assert(NCH <= BF_NCS || NCH % BF_NCS == 0, "matrix ring: chunks per tile must tile the ring");
     if (warp == 0) {
         // [ledger: a11 matrix stream (TMA bulk copies)]
         // ------------------------------------------------ matrix producer (whole warp walks the loop, one lane issues)
-        uint32_t m = 0;
-        for (long long pit = 0, tile; (tile = bf_tile(pit)) < ntiles; pit++) {
+        for (uint32_t pit = 0; bf_tile(pit) < ntiles; pit++) {
             int tb, ts, to;
-            tile_coords_pow2(g, tile, lg_nbt, lg_ns, tb, ts, to);
+            tile_coords_pow2(g, bf_tile(pit), lg_nbt, lg_ns, tb, ts, to);
             const uint8_t *mb = mat + (size_t)(g.matsel ? ts : 0) * bf_mat_bytes(K);
-            for (int c = 0; c < 2 * NCH; c++, m++) {
-                const uint32_t slot = m % BF_NSLOT, use = m / BF_NSLOT;
-                if (use) bf_wait(&b_empty[slot], (use - 1) & 1);
+#pragma unroll
+            for (int ch = 0; ch < NCH; ch++) {  // one copy per chunk: its two parity blocks are adjacent in the table
+                const int cs = ch % BF_NCS;
+                const uint32_t use = UPT * pit + ch / BF_NCS;  // how often this ring entry has been filled before
+                if (use) bf_wait_slack(&b_empty[cs], (use - 1) & 1);
                 if (elect_one()) {
-                    mbar_expect_tx(&b_full[slot], SB);
-                    bulk_g2s(sB + slot * SB, mb + (size_t)c * SB, SB, &b_full[slot]);
+                    mbar_expect_tx(&b_full[cs], 2 * SB);
+                    bulk_g2s(sB + cs * 2 * SB, mb + (size_t)ch * 2 * SB, 2 * SB, &b_full[cs]);
                 }
                 __syncwarp();
             }
@@ -229,63 +250,106 @@ __global__ void __launch_bounds__(BF_THREADS, 1) stage_bf_kernel(StageGeom g, co
         // ------------------------------------------------ tensor-core issuer (one elected lane; program order = execution order)
         // per tile: tcgen05.cp of the data operand shared memory -> TMEM (then the shared copy is free for the next
         // tile); per chunk: a4 stage MMAs with A from TMEM (a3 and a5 folded into the operands), then a6 Phase A with
-        // A = the stage accumulators.  Every descriptor is one base plus a compile-time constant.
+        // A = the stage accumulators.  This warp's instruction stream paces the tensor pipe (ncu: the pipe idles while the
+        // issuer works through waits and address set-up), so the stream is kept short: the chunk loop is unrolled (ring
+        // slots and barrier parities are constants), and one elected region per chunk issues Phase A of the PREVIOUS chunk
+        // followed by the stage MMAs of this one -- the same program order as chunk-by-chunk issue, a quarter of the
+        // wait / elect / reconverge sequences.
         const uint32_t idesc_st = make_idesc(CFMT_S32, I8_U8, I8_U8, 128, BF_N), idesc_pa = make_idesc(CFMT_S32, I8_U8, I8_U8, 128, 32);
         const uint64_t bdesc0 = make_sdesc(smem_u32(sB), BF_N * 16, 128), pdesc0 = make_sdesc(smem_u32(sPA), 32 * 16, 128);
         const uint64_t adesc0 = make_sdesc(smem_u32(sA), BF_COLS * 16, 128);
         constexpr int ACOLS = 3 * NCK * 4;  // TMEM columns of one parity of the data operand
-        uint32_t m = 0, n = 0, it = 0;
-        for (long long tile; (tile = bf_tile(it)) < ntiles; it++) {
-            bf_wait(&a_full[0], it & 1);
-            tc_fence_after();
-            if (elect_one()) {
+        // the TMEM base (0) as a value of the uniform datapath that the compiler cannot fold or hoist: every TMEM address
+        // below is then one uniform add next to its use, not a constant built in a vector register and moved across
+        const uint32_t tz0 = (uint32_t)g.K >> 16;
+        auto tzero = [&]() { uint32_t z; asm volatile("mov.u32 %0, %1;" : "=r"(z) : "r"(tz0)); return z; };
+        auto opaque64 = [](uint64_t v) { uint64_t z; asm volatile("mov.b64 %0, %1;" : "=l"(z) : "l"(v)); return z; };  // same for descriptors
+        uint32_t it = 0;
+        uint32_t gc = 0;  // Phase-A unit -> epilogue group (round robin)
+        bool pend = false;                           // Phase A of the last issued chunk is still to be issued
+#ifdef OZFFT_PIPE_TIMERS
+        long long dbg_[8] = {0, 0, 0, 0, 0, 0, 0, 0};
+        const long long tstart_ = clock64();
+#endif
+        // Phase A of chunk number j (counted over the launch) needs the two D_PA slots back from chunk j - 1: one barrier,
+        // eight arrivals (two units x four warps)
+        uint32_t npa = 0;  // chunks whose Phase A has been issued
+        auto wait_pa = [&]() {
+            if (npa) { OZ_T0(); bf_wait(&pa_empty[0], (npa - 1) & 1); OZ_T1(2); }
+            npa++;
+        };
+        auto issue_pa = [&](uint32_t g0, uint32_t g1) {  // elected lane only
+            const uint32_t tz = tzero();
+            const uint64_t pdz = opaque64(pdesc0);
 #pragma unroll
-                for (int par = 0; par < 2; par++)
+            for (int gg = 0; gg < 2; gg++) {
 #pragma unroll
-                    for (int pl = 0; pl < 3; pl++)
+                for (int P = 0; P < 2; P++)
 #pragma unroll
-                        for (int t = 0; t < NCK; t++)
-                            tmem_cp_128x128b(tmem + BF_TA + par * ACOLS + (pl * NCK + t) * 4,
-                                             adesc0 + (uint64_t)((pl * PLANE + par * PARB + t * (BF_COLS * 16)) >> 4));
-                tc_commit(&a_empty[0]);
+                    for (int s = 0; s < 6; s++)
+                        mma_i8_ts(tz + (BF_DPA + gg * 64 + P * 32), tz + (BF_TD + P * 96 + (s >= 3 ? 48 : 0) + gg * 24 + (s % 3) * 8),
+                                  pdz + (uint64_t)((s * 2 * 32 * 16) >> 4), idesc_pa, s > 0);
+                tc_commit(&pa_full[gg ? g1 : g0]);
             }
-            __syncwarp();
-            for (int ch = 0; ch < NCH; ch++, n++) {
+        };
+        for (; bf_tile(it) < ntiles; it++) {
 #pragma unroll
-                for (int par = 0; par < 2; par++, m++) {
-                    const uint32_t slot = m % BF_NSLOT;
-                    bf_wait(&b_full[slot], (m / BF_NSLOT) & 1);
-                    tc_fence_after();
-                    if (elect_one()) {
-                        const uint64_t bd = bdesc0 + (uint64_t)((slot * SB) >> 4);
+            for (int ch = 0; ch < NCH; ch++) {
+                const uint32_t g0 = gc, g1 = gc + 1 == BF_NG ? 0 : gc + 1;
+                if (pend) wait_pa();
+                if (ch == 0) {  // tile boundary: Phase A of the previous tile's last chunk goes out before the wait for the new operand
+                    if (pend) {
+                        tc_fence_after();
+                        if (elect_one()) issue_pa(g0, g1);
+                        __syncwarp();
+                    }
+                    { OZ_T0(); bf_wait(&a_full[0], it & 1); OZ_T1(0); }
+                }
+                { OZ_T0(); bf_wait(&b_full[ch % BF_NCS], (UPT * it + ch / BF_NCS) & 1); OZ_T1(1); }
+                tc_fence_after();
+                if (elect_one()) {
+                    const uint32_t tz = tzero();
+                    const uint64_t bdz = opaque64(bdesc0), adz = opaque64(adesc0);
+                    if (ch == 0) {
+#pragma unroll
+                        for (int par = 0; par < 2; par++)
+#pragma unroll
+                            for (int pl = 0; pl < 3; pl++)
+#pragma unroll
+                                for (int t = 0; t < NCK; t++)
+                                    tmem_cp_128x128b(tz + (BF_TA + par * ACOLS + (pl * NCK + t) * 4),
+                                                     adz + (uint64_t)((pl * PLANE + par * PARB + t * (BF_COLS * 16)) >> 4));
+                        tc_commit(&a_empty[0]);
+                    } else if (pend) {
+                        issue_pa(g0, g1);
+                    }
+#pragma unroll
+                    for (int par = 0; par < 2; par++) {
+                        const uint64_t bd = bdz + (uint64_t)((((ch % BF_NCS) * 2 + par) * SB) >> 4);
 #pragma unroll
                         for (int P = 0; P < 2; P++)  // P = 0: re rows [XR ; NXI] (planes 1, 2), P = 1: im rows [XI ; XR] (planes 0, 1)
 #pragma unroll
                             for (int s = 0; s < NCK; s++)  // K step s = chunks 2s, 2s+1 of the two adjacent planes
-                                mma_i8_ts(tmem + BF_TD + P * 96 + par * 48, tmem + BF_TA + par * ACOLS + ((1 - P) * NCK + 2 * s) * 4,
+                                mma_i8_ts(tz + (BF_TD + P * 96 + par * 48), tz + (BF_TA + par * ACOLS + ((1 - P) * NCK + 2 * s) * 4),
                                           bd + (uint64_t)((s * 2 * BF_N * 16) >> 4), idesc_st, s > 0);
-                        tc_commit(&b_empty[slot]);
                     }
-                    __syncwarp();
+                    tc_commit(&b_empty[ch % BF_NCS]);
                 }
-#pragma unroll
-                for (int gg = 0; gg < 2; gg++) {
-                    const uint32_t u = 2 * n + gg;  // unit index; its D_PA slot gg was last used by unit u - 2
-                    if (u >= 2) bf_wait(&pa_empty[(u - 2) % 3], ((u - 2) / 3) & 1);
-                    tc_fence_after();
-                    if (elect_one()) {
-#pragma unroll
-                        for (int P = 0; P < 2; P++)
-#pragma unroll
-                            for (int s = 0; s < 6; s++)
-                                mma_i8_ts(tmem + BF_DPA + gg * 64 + P * 32, tmem + BF_TD + P * 96 + (s >= 3 ? 48 : 0) + gg * 24 + (s % 3) * 8,
-                                          pdesc0 + (uint64_t)((s * 2 * 32 * 16) >> 4), idesc_pa, s > 0);
-                        tc_commit(&pa_full[u % 3]);
-                    }
-                    __syncwarp();
-                }
+                __syncwarp();
+                if (pend) gc = g1 + 1 == BF_NG ? 0 : g1 + 1;
+                pend = true;
             }
         }
+        if (pend) {  // Phase A of the very last chunk
+            const uint32_t g0 = gc, g1 = gc + 1 == BF_NG ? 0 : gc + 1;
+            wait_pa();
+            tc_fence_after();
+            if (elect_one()) issue_pa(g0, g1);
+            __syncwarp();
+        }
+#ifdef OZFFT_PIPE_TIMERS
+        if (lane == 0) { dbg_[3] = clock64() - tstart_; dbg_[4] = it; for (int i = 0; i < 8; i++) g_bf_dbg[blockIdx.x][i] = dbg_[i]; }
+#endif
     } else if (warp >= 4 && warp < 12) {
         // [ledger: a1 load + addressing]
         // ------------------------------------------------ deconstruction: thread = (column, parity of j)
@@ -296,9 +360,8 @@ __global__ void __launch_bounds__(BF_THREADS, 1) stage_bf_kernel(StageGeom g, co
             const uint32_t buf = it & 1;
             int tb, ts, to;
             tile_coords_pow2(g, tile, lg_nbt, lg_ns, tb, ts, to);
-            const int blk = 4 * tb + (c >> 5);
-            const bool valid = blk * 32 + (c & 31) < g.ncols;
-            const uint4 *src = in + ((long long)blk * g.ib + (long long)ts * g.is + (long long)to * g.io + (long long)(c & 31) * g.lane + (long long)par * g.ji);
+            const bool valid = tb * BF_COLS + c < g.ncols;
+            const uint4 *src = in + (col_off(g.ci, tb, c) + (long long)ts * g.is + (long long)to * g.io + (long long)par * g.ji);
             const long long jstep = 2 * g.ji;
             // [ledger: a2 column exponent]
             // a2: column exponent = max of the 11-bit exponent fields (integer compare on the high words)
@@ -379,16 +442,19 @@ __global__ void __launch_bounds__(BF_THREADS, 1) stage_bf_kernel(StageGeom g, co
         const int qd = (warp - 12) >> 2, row = (warp & 3) * 32 + lane;
         const uint32_t lane_taddr = tmem + ((uint32_t)((warp & 3) * 32) << 16);
         uint32_t it = 0, nu = 0;  // tiles seen, units this group has consumed
-        int turn = qd;            // units to skip until the next one of this group (units go round-robin over the 3 groups)
+#ifdef OZFFT_PIPE_TIMERS
+        long long dbg_[8] = {0, 0, 0, 0, 0, 0, 0, 0};
+        const long long tstart_ = clock64();
+#endif
+        int turn = qd;            // units to skip until the next one of this group (units go round-robin over the groups)
         for (long long tile; (tile = bf_tile(it)) < ntiles; it++) {
             const uint32_t buf = it & 1;
             int tb, ts, to;
             tile_coords_pow2(g, tile, lg_nbt, lg_ns, tb, ts, to);
-            const int blk = 4 * tb + (row >> 5);
-            const bool valid = blk * 32 + (row & 31) < g.ncols;
-            uint4 *dstp = out + ((long long)blk * g.ob + (long long)ts * g.os + (long long)to * g.oo + (long long)(row & 31) * g.olane);
+            const bool valid = tb * BF_COLS + row < g.ncols;
+            uint4 *dstp = out + (col_off(g.co, tb, row) + (long long)ts * g.os + (long long)to * g.oo);
             const uint4 *ct = ctab + (size_t)(g.matsel ? ts : 0) * K;
-            bf_wait_slack(&a_full[0], it & 1);  // the column exponents of this tile are published (s_T is double buffered: the
+            { OZ_T0(); bf_wait_slack(&a_full[0], it & 1); OZ_T1(6); }  // the column exponents of this tile are published (s_T is double buffered: the
             const int Tmax = s_T[buf][row], flag = s_flag[buf][row];  // deconstruction runs at most one tile ahead)
             __syncwarp();
             if (lane == 0) mbar_arrive(&e_start[0]);
@@ -399,13 +465,13 @@ __global__ void __launch_bounds__(BF_THREADS, 1) stage_bf_kernel(StageGeom g, co
 #pragma unroll 1
                 for (int gg = 0; gg < 2; gg++) {
                     if (turn) { turn--; continue; }
-                    turn = 2;
+                    turn = BF_NG - 1;
                     const int kp = 2 * ch + gg;
                     uint4 cc[2];
                     cc[0] = __ldg(ct + (kp < H ? kp : 0));
                     cc[1] = __ldg(ct + (kp < H ? kp + H : 0));
                     // [ledger: a7 Phase B deposits (TMEM loads, slice sums -> E)]
-                    bf_wait_slack(&pa_full[qd], nu & 1);
+                    { OZ_T0(); bf_wait_pa(&pa_full[qd], nu & 1); OZ_T1(5); }
                     tc_fence_after();
                     uint32_t E[4][5];  // [part*2 + o]
 #pragma unroll
@@ -417,25 +483,24 @@ __global__ void __launch_bounds__(BF_THREADS, 1) stage_bf_kernel(StageGeom g, co
                     }
                     tc_fence_before();
                     __syncwarp();
-                    if (lane == 0) mbar_arrive(&pa_empty[qd]);
+                    if (lane == 0) mbar_arrive(&pa_empty[0]);
                     nu++;
                     if (kp >= H || !valid) continue;
                     // [ledger: a12 store + addressing]
                     uint4 *dk = dstp + (long long)kp * g.ko;
                     if (flag == 1) {  // the usual column: finite, not all zero
+                        // a8 lift + a9 pack of the four outputs as one straight-line block (finish_fast); the rare outputs that
+                        // need the two-sided correction, are tiny against the column scale or leave the normal range are redone
+                        uint64_t y[4];
 #pragma unroll
-                        for (int o = 0; o < 2; o++) {
-                            uint64_t y[2];
-#pragma unroll
-                            for (int P = 0; P < 2; P++) {
-                                const uint32_t *e = E[P * 2 + o];
-                                uint32_t r[4], r2[4];
-                                crt_from_E(e[0], e[1], e[2], e[3], e[4], r);                        // a8: lift, two-sided centring
-                                sub128(r2, r[0], r[1], r[2], r[3], cc[o].x, cc[o].y, cc[o].z, cc[o].w);  // minus the offset constant
-                                y[P] = pack_limbs(r2, gexp);                                        // a9: one rounding to fp64
-                            }
-                            dk[o * hko] = make_uint4((uint32_t)y[0], (uint32_t)(y[0] >> 32), (uint32_t)y[1], (uint32_t)(y[1] >> 32));  // a12
+                        for (int x = 0; x < 4; x++) {
+                            uint32_t r[4], r2[4];
+                            crt_from_E(E[x][0], E[x][1], E[x][2], E[x][3], E[x][4], r);
+                            sub128(r2, r[0], r[1], r[2], r[3], cc[x & 1].x, cc[x & 1].y, cc[x & 1].z, cc[x & 1].w);
+                            y[x] = pack_limbs(r2, gexp);
                         }
+                        dk[0] = make_uint4((uint32_t)y[0], (uint32_t)(y[0] >> 32), (uint32_t)y[2], (uint32_t)(y[2] >> 32));    // a12: out k
+                        dk[hko] = make_uint4((uint32_t)y[1], (uint32_t)(y[1] >> 32), (uint32_t)y[3], (uint32_t)(y[3] >> 32));  //      out k + H
                     } else {  // all-zero column -> +0, non-finite column -> NaN (reading S18)
                         const uint32_t hi = (flag & 2) ? 0x7FF80000u : 0u;
                         dk[0] = make_uint4(0, hi, 0, hi);
@@ -443,6 +508,9 @@ __global__ void __launch_bounds__(BF_THREADS, 1) stage_bf_kernel(StageGeom g, co
                     }
                 }
         }
+#ifdef OZFFT_PIPE_TIMERS
+        if (warp == 12 && lane == 0) { g_bf_dbg[blockIdx.x][5] = dbg_[5]; g_bf_dbg[blockIdx.x][6] = dbg_[6]; g_bf_dbg[blockIdx.x][7] = clock64() - tstart_; }
+#endif
     }
     // [ledger: setup, tile decode, loop control]
     tc_fence_before();

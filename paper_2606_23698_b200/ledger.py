@@ -1,6 +1,6 @@
 """Epilogue instruction ledger by term (PAPER.md:437-445 table, 558 eps_mix, 876, 890).
 
-  python -m paper_2606_23698_b200.ledger REPORT.ncu-rep --n-out N [--md OUT.md] [--lines OUT.csv]
+  python -m paper_2606_23698_b200.ledger REPORT.ncu-rep --n-out N [--launch I] [--md OUT.md] [--lines OUT.csv]
   python -m paper_2606_23698_b200.ledger --static            # SASS opcode histogram of the built library
 
 REPORT is one `ncu --set full --import-source on` capture of ONE stage-kernel launch (the recipe in
@@ -72,7 +72,12 @@ def term_of(tmap, fname, line):
     return t
 
 
+LAUNCH = 0  # which launch of a multi-launch report to read (--launch)
+
+
 def _ncu(args):
+    if args[:1] == ["-i"]:
+        args = args[:2] + ["--launch-skip", str(LAUNCH), "--launch-count", "1"] + args[2:]
     r = subprocess.run(["ncu"] + args, capture_output=True, text=True)
     if r.returncode != 0:
         raise SystemExit("ncu failed: " + r.stderr[-2000:])
@@ -208,8 +213,11 @@ def main():
     ap.add_argument("--n-out", type=float)
     ap.add_argument("--md", help="write the tables to this file as well")
     ap.add_argument("--lines", help="write the per-line counts (file, line, term, thread inst, predicated-on) as CSV")
+    ap.add_argument("--launch", type=int, default=0, help="index of the launch to read in a report that holds several (default 0)")
     ap.add_argument("--static", action="store_true", help="SASS opcode histogram of libozfft.so (no report needed)")
     a = ap.parse_args()
+    global LAUNCH
+    LAUNCH = a.launch
     if a.static:
         out = static_histogram(os.path.join(_HERE, "libozfft.so"))
     else:
