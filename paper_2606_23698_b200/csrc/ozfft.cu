@@ -51,6 +51,8 @@ struct StageLaunch {
     const uint8_t *mat_f8;    // E4M3 hex-digit planes of the FP8 rung (stage_f8.cuh)
     const void *ctab_bf;      // its offset constants [nmat][K] x 16 B
     int axis;
+    bool fused;               // byte-fed kernel, axis of length 1024: both stages in one launch (stage_bf.cuh BfFuse); g = first stage
+    BfFuse fuse;              // second stage and group layout (ring and counters are filled in at launch from the plan)
 };
 
 }  // namespace
@@ -69,6 +71,10 @@ struct ozfft_plan_s {
     size_t dev_bytes;
     DevConsts *d_consts;
     void *work;
+    void *ring;           // fused axes: Y' ring (L2 resident) and the group counters
+    unsigned int *ctr;
+    int ring_slots, fuse_lag, max_groups;
+    bool fuse;            // schedule: fused axes where the shape allows (OZFFT_SCHEDULE=unfused turns it off)
     void *h_in, *h_out;  // device staging for ozfft_exec_host (lazy)
     bool pipelined;      // exec_host overlaps the copies with the passes
     std::vector<StageLaunch> slab_stages;  // z and y stages of one slab of nx/PIPE planes
@@ -197,7 +203,7 @@ struct AxisDesc {
 
 // perm_out: the second stage of this (contiguous) axis writes index k1 + p k2 instead of k2 + 32 k1; unperm = p > 0: the first
 // stage of this axis reads an inner index permuted that way and writes the natural one (StageGeom::patch)
-bool add_axis(ozfft_plan_s *p, const AxisDesc &a, int axis, MatMap &mats, std::vector<StageLaunch> &dst, bool perm_out = false, int unperm = 0) {
+bool add_axis(ozfft_plan_s *p, const AxisDesc &a, int axis, MatMap &mats, std::vector<StageLaunch> &dst, bool perm_out = false, int unperm = 0, bool fuse = false) {
     const int N = (int)a.N;
     const bool two = N > 32;
     const int q = two ? 32 : N, pp = two ? N / 32 : 1;
@@ -284,6 +290,42 @@ bool add_axis(ozfft_plan_s *p, const AxisDesc &a, int axis, MatMap &mats, std::v
         g1.co = StageGeom::ColMap{1, 1, 7, 3, 256, 16, 32, 1};
     }
     if (!get(q, 0, s1)) return false;
+    const long long cols = a.contiguous ? a.outer : a.inner;  // columns along the b coordinate
+    if (fuse && p->variant == 2 && two && pp == 32 && cols % 128 == 0) {
+        // fused axis: Y' of a group of 128 pencils (32 x 4096 elements) lives in a ring slot, laid out [k2][j1 or pencil][...]
+        if (!get(pp, N, s2)) return false;
+        StageLaunch sf = s1;
+        sf.fused = true;
+        BfFuse &f = sf.fuse;
+        f = BfFuse{};
+        f.g2 = g2;
+        f.mat2 = s2.mat_bf;
+        f.ctab2 = (const uint4 *)s2.ctab_bf;
+        if (unperm) f.g2.co = g1.co;  // the group's 128 columns are the 8 x 16 patch: the second stage stores them at their natural places
+        sf.g.os = 0; sf.g.oo = 0; sf.g.ko = 4096;
+        f.g2.is = 4096; f.g2.io = 0;
+        if (a.contiguous) {  // first-stage tile = 4 pencils x 32 j1 -> ring [k2][pencil][j1]; second-stage column = pencil
+            sf.g.co = StageGeom::ColMap{0, 0, 127, 7, 128, 0, 1, 0};
+            f.g2.ci = StageGeom::ColMap{0, 0, 127, 7, 0, 0, 32, 0};
+            f.g2.ji = 1;
+            f.G = (int)(cols / 128);
+            f.lg_nbt = 30;
+            f.s1_mulb = 32; f.s1_tlb = 1; f.s1_tls = 0; f.r1_tlb = 1; f.r1_tls = 0;
+        } else {             // first-stage tile = one j1 of 128 lanes -> ring [k2][j1][lane]
+            sf.g.co = StageGeom::ColMap{0, 0, 127, 7, 0, 0, 1, 0};
+            sf.g.os = 128;
+            f.g2.ci = StageGeom::ColMap{0, 0, 127, 7, 0, 0, 1, 0};
+            f.g2.ji = 128;
+            const int nbt = (int)(cols / 128);
+            f.G = nbt * (int)a.outer;
+            f.lg_nbt = 0;
+            while ((1 << f.lg_nbt) < nbt) f.lg_nbt++;
+            f.s1_mulb = 1; f.s1_tlb = 0; f.s1_tls = 1; f.r1_tlb = 0; f.r1_tls = 1;
+        }
+        if (f.G > p->max_groups) p->max_groups = f.G;
+        dst.push_back(sf);
+        return true;
+    }
     dst.push_back(s1);
     if (two) {
         if (!get(pp, N, s2)) return false;
@@ -316,6 +358,15 @@ ozfft_plan_s *make_plan(int nx, int ny, int nz, int sign, bool batched1d) {
     p->variant = pick_variant();
     p->dev_bytes = 0;
     p->work = p->h_in = p->h_out = nullptr;
+    p->ring = nullptr; p->ctr = nullptr; p->max_groups = 0;
+    {   // schedule of the byte-fed kernel: axes of length 1024 run both stages in one launch unless OZFFT_SCHEDULE=unfused
+        const char *sch = getenv("OZFFT_SCHEDULE");
+        p->fuse = !(sch && !strcmp(sch, "unfused"));
+        // lag 8 groups, ring 14 slots = 28 MB (measured at 1024^3: lag 3 / 4 / 6 / 8 / 12 -> 191 / 144 / 131 / 130 / 132 ms: below ~6 the
+        // second-stage tiles catch up with the first-stage tiles still in flight on the 148 SMs and wait)
+        p->fuse_lag = 8;
+        p->ring_slots = 14;
+    }
     p->pipelined = false;
     p->s_in = p->s_out = nullptr;
     DevConsts hc;
@@ -334,14 +385,17 @@ ozfft_plan_s *make_plan(int nx, int ny, int nz, int sign, bool batched1d) {
         ok = p->pa_bf != nullptr;
     }
     if (batched1d) {  // nx = batch, nz = n
-        ok = ok && add_axis(p, AxisDesc{true, nx, nz, 1}, 0, mats, p->stages);
+        ok = ok && add_axis(p, AxisDesc{true, nx, nz, 1}, 0, mats, p->stages, false, 0, p->fuse);
+        if (ok && !p->stages.empty() && p->stages[0].fused) ok = add_axis(p, AxisDesc{true, nx, nz, 1}, 0, mats, p->stages_nat);
     } else {
         // byte-fed kernel, nz >= 256: the z pass leaves its output permuted along z and the first y stage undoes it (stage.cuh)
         const bool perm = p->variant == 2 && nz >= 256;
-        ok = ok && add_axis(p, AxisDesc{true, (long long)nx * ny, nz, 1}, 0, mats, p->stages, perm, 0);
-        ok = ok && add_axis(p, AxisDesc{false, nx, ny, nz}, 1, mats, p->stages, false, perm ? nz / 32 : 0);
-        ok = ok && add_axis(p, AxisDesc{false, 1, nx, (long long)ny * nz}, 2, mats, p->stages);
-        if (perm) {
+        ok = ok && add_axis(p, AxisDesc{true, (long long)nx * ny, nz, 1}, 0, mats, p->stages, perm, 0, p->fuse);
+        ok = ok && add_axis(p, AxisDesc{false, nx, ny, nz}, 1, mats, p->stages, false, perm ? nz / 32 : 0, p->fuse);
+        ok = ok && add_axis(p, AxisDesc{false, 1, nx, (long long)ny * nz}, 2, mats, p->stages, false, 0, p->fuse);
+        bool any_fused = false;
+        for (const StageLaunch &sl : p->stages) any_fused = any_fused || sl.fused;
+        if (perm || any_fused) {
             ok = ok && add_axis(p, AxisDesc{true, (long long)nx * ny, nz, 1}, 0, mats, p->stages_nat);
             ok = ok && add_axis(p, AxisDesc{false, nx, ny, nz}, 1, mats, p->stages_nat);
             ok = ok && add_axis(p, AxisDesc{false, 1, nx, (long long)ny * nz}, 2, mats, p->stages_nat);
@@ -358,6 +412,11 @@ ozfft_plan_s *make_plan(int nx, int ny, int nz, int sign, bool batched1d) {
     if (ok) {
         ok = cuda_ok(cudaMalloc(&p->work, (size_t)p->count * 16), "cudaMalloc(workspace)");
         if (ok) p->dev_bytes += (size_t)p->count * 16;
+    }
+    if (ok && p->max_groups) {  // fused axes: the Y' ring and two counters per group
+        const size_t rb = (size_t)p->ring_slots * BF_GROUP_ELEMS * 16, cb = (size_t)p->max_groups * 8;
+        ok = cuda_ok(cudaMalloc(&p->ring, rb), "cudaMalloc(ring)") && cuda_ok(cudaMalloc((void **)&p->ctr, cb), "cudaMalloc(counters)");
+        if (ok) p->dev_bytes += rb + cb;
     }
     // per plan, on the plan's device: kernel attributes and the constant bank (both are per-device state)
     if (ok && (p->variant == 0 || p->variant == 3 || p->variant == 4)) {
@@ -393,6 +452,17 @@ int launch_stage(ozfft_plan p, const StageLaunch &s, const void *src, void *dst,
     const long long nt = (long long)s.g.nb * s.g.ns * s.g.no;
     if (p->variant == 5) {
         return cuda_ok(stage_f8_launch(s.g, src, dst, s.mat_f8, p->sms, st), "stage_f8_kernel launch") ? OZFFT_OK : OZFFT_ECUDA;
+    }
+    if (p->variant == 2 && s.fused) {
+        BfFuse f = s.fuse;
+        f.ring = (uint4 *)p->ring;
+        f.wr_done = p->ctr;
+        f.rd_done = p->ctr + p->max_groups;
+        f.Lg = p->fuse_lag < f.G ? p->fuse_lag : f.G;
+        f.R = p->ring_slots;
+        if (stage_bf_launch_fused(s.g, f, src, dst, s.mat_bf, s.ctab_bf, p->pa_bf, p->sms, st)) return OZFFT_OK;
+        set_err(std::string("stage_bf_kernel (fused axis) launch: ") + cudaGetErrorString(cudaGetLastError()));
+        return OZFFT_ECUDA;
     }
     if (p->variant == 2) {
         if (stage_bf_launch(s.g, src, dst, s.mat_bf, s.ctab_bf, p->pa_bf, p->sms, st)) return OZFFT_OK;
@@ -483,7 +553,8 @@ static int exec_host_pipelined_body(ozfft_plan p, const char *hin, char *hout, c
         }
         if (!cuda_ok(cudaEventCreateWithFlags(&p->ev_start, cudaEventDisableTiming), "cudaEventCreate")) return OZFFT_ECUDA;
     }
-    const size_t L = p->stages.size(), Lzy = p->slab_stages.size();
+    const std::vector<StageLaunch> &full = p->stages_nat.empty() ? p->stages : p->stages_nat;  // stage by stage (the x pass runs per chunk)
+    const size_t L = full.size(), Lzy = p->slab_stages.size();
     auto buf_of = [&](size_t i) -> char * { return (char *)(((L - 1 - i) & 1) ? p->work : p->h_out); };  // as run_stages
     // copies start once earlier work on the caller's stream is done
     if (!cuda_ok(cudaEventRecord(p->ev_start, st), "cudaEventRecord") || !cuda_ok(cudaStreamWaitEvent(p->s_in, p->ev_start, 0), "cudaStreamWaitEvent") ||
@@ -506,7 +577,7 @@ static int exec_host_pipelined_body(ozfft_plan p, const char *hin, char *hout, c
         const size_t off = (size_t)(c * yc * nz) * 16;
         const char *src = (Lzy ? buf_of(Lzy - 1) : (char *)p->h_in) + off;
         for (size_t i = Lzy; i < L; i++) {
-            StageLaunch sl = p->stages[i];
+            StageLaunch sl = full[i];
             sl.g.nb = (int)(yc * nz / 32);
             sl.g.ncols = (int)(yc * nz);
             char *dst = buf_of(i) + off;
@@ -561,6 +632,8 @@ void ozfft_plan_destroy(ozfft_plan p) {
     }
     for (void *d : p->dev_allocs) cudaFree(d);
     if (p->work) cudaFree(p->work);
+    if (p->ring) cudaFree(p->ring);
+    if (p->ctr) cudaFree(p->ctr);
     if (p->h_in) cudaFree(p->h_in);
     if (p->h_out) cudaFree(p->h_out);
     if (p->s_in) {

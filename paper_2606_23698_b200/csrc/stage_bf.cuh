@@ -185,11 +185,79 @@ __device__ __forceinline__ void bf_append7(uint32_t *wd, int e, uint32_t lo, uin
     }
 }
 
+// ---------------------------------------------------------------------------------------------------- fused axis
+// Both stages of one axis of length 1024 in ONE launch (beta -> 1; Alg. 1 lines 7-8).
+// The paper keeps Y' of one transform on chip; a tcgen05 tile here is 128 columns that share one matrix, so the unit of
+// fusion is a GROUP of 128 pencils: 32 first-stage tiles (4 pencils x 32 j1 each, or one j1 of 128 lanes) followed by 32
+// second-stage tiles (one k2 each), with Y' of the group (2 MB) in a ring of R slots that stays in the 126 MB L2 -- it is
+// written once, read once and overwritten before it is evicted, so it never reaches HBM.  The persistent CTAs walk one
+// tile sequence in which a group's second stage comes `Lg` groups after its first stage; a second-stage tile waits (global
+// counter, acquire) until all first-stage tiles of its group have stored, a first-stage tile until the ring slot it will
+// overwrite has been read.  Every wait is on tiles earlier in the sequence, and all CTAs are resident: no deadlock.
+struct BfFuse {
+    StageGeom g2;                  // second stage: input side = ring (compact), output side = the axis output
+    const uint8_t *mat2;           // its 32 twiddle-fused matrices (Eq. 6)
+    const uint4 *ctab2;
+    uint4 *ring;                   // R slots x 131072 elements
+    unsigned int *wr_done, *rd_done;  // per group: first-stage (warp, unit) stores done; second-stage warps done reading
+    int G, Lg, R;                  // groups, lag, ring slots (R > Lg)
+    int lg_nbt;                    // group = (go << lg_nbt) | gb
+    int s1_mulb, s1_tlb, s1_tls;   // first-stage input tile: tb = gb * s1_mulb + tl * s1_tlb, ts = tl * s1_tls, to = go
+    int r1_tlb, r1_tls;            // first-stage output (ring) tile: tb = tl * r1_tlb, ts = tl * r1_tls
+};
+constexpr int BF_GROUP_ELEMS = 32 * 4096;          // Y' of one group
+constexpr unsigned BF_WR_TARGET = 32 * 16 * 4;     // first-stage tiles x units x warps per unit
+constexpr unsigned BF_RD_TARGET = 32 * 8;          // second-stage tiles x deconstruction warps
+
+struct BfLoc { int st, grp, tl, tbi, tsi, toi, tbo, tso, too; };
+
+template <bool FUSED>
+__device__ __forceinline__ BfLoc bf_locate(const StageGeom &g, const BfFuse &f, long long tile, int lg_nbt, int lg_ns) {
+    BfLoc L;
+    if (!FUSED) {
+        int tb, ts, to;
+        tile_coords_pow2(g, tile, lg_nbt, lg_ns, tb, ts, to);
+        L.st = 0; L.grp = 0; L.tl = 0;
+        L.tbi = L.tbo = tb; L.tsi = L.tso = ts; L.toi = L.too = to;
+        return L;
+    }
+    const int q = (int)(tile >> 5), Lg = f.Lg, G = f.G;
+    L.tl = (int)tile & 31;
+    if (q < Lg) { L.st = 0; L.grp = q; }
+    else {
+        const int r = q - Lg;
+        if (r < 2 * (G - Lg)) { L.st = r & 1; L.grp = L.st ? (r >> 1) : Lg + (r >> 1); }
+        else { L.st = 1; L.grp = G - Lg + (r - 2 * (G - Lg)); }
+    }
+    const int gb = L.grp & ((1 << f.lg_nbt) - 1), go = L.grp >> f.lg_nbt;
+    if (L.st == 0) { L.tbi = gb * f.s1_mulb + L.tl * f.s1_tlb; L.tsi = L.tl * f.s1_tls; L.toi = go; L.tbo = L.tl * f.r1_tlb; L.tso = L.tl * f.r1_tls; L.too = 0; }
+    else { L.tbi = 0; L.tsi = L.tl; L.toi = 0; L.tbo = gb; L.tso = L.tl; L.too = go; }
+    return L;
+}
+
+// loads of the stage input: read-only path, or L2-coherent (the ring is written by other SMs during the launch)
+template <bool FUSED> __device__ __forceinline__ uint4 bf_ld(const uint4 *p) {
+    if (!FUSED) return __ldg(p);
+    uint4 v;
+    asm volatile("ld.global.cg.v4.u32 {%0,%1,%2,%3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "l"(p));
+    return v;
+}
+// wait until a global counter reaches `target` (acquire; bounded: a protocol bug must trap, not hang)
+__device__ __forceinline__ void bf_wait_global(const unsigned int *ctr, unsigned int target) {
+    unsigned int v, spins = 0;
+    for (;;) {
+        asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(ctr) : "memory");
+        if (v >= target) break;
+        if (++spins > (1u << 24)) __trap();
+        __nanosleep(200);
+    }
+}
+
 // [ledger: setup, tile decode, loop control]
-template <int K>
+template <int K, bool FUSED>
 __global__ void __launch_bounds__(BF_THREADS, 1) stage_bf_kernel(StageGeom g, const uint4 *__restrict__ in, uint4 *__restrict__ out,
                                                                  const uint8_t *__restrict__ mat, const uint4 *__restrict__ ctab,
-                                                                 const uint4 *__restrict__ pa_g, long long ntiles) {
+                                                                 const uint4 *__restrict__ pa_g, long long ntiles, BfFuse f) {
     constexpr int H = bf_H(K), PB = bf_PB(K), NCK = bf_NCK(K), NCH = bf_NCH(K);
     constexpr int SB = bf_slot_bytes(K), PLANE = bf_plane_bytes(K), ASET = bf_aset_bytes(K), PARB = NCK * BF_COLS * 16;
     constexpr int NW = PB / 4;
@@ -230,9 +298,8 @@ __global__ void __launch_bounds__(BF_THREADS, 1) stage_bf_kernel(StageGeom g, co
         // [ledger: a11 matrix stream (TMA bulk copies)]
         // ------------------------------------------------ matrix producer (whole warp walks the loop, one lane issues)
         for (uint32_t pit = 0; bf_tile(pit) < ntiles; pit++) {
-            int tb, ts, to;
-            tile_coords_pow2(g, bf_tile(pit), lg_nbt, lg_ns, tb, ts, to);
-            const uint8_t *mb = mat + (size_t)(g.matsel ? ts : 0) * bf_mat_bytes(K);
+            const BfLoc L = bf_locate<FUSED>(g, f, bf_tile(pit), lg_nbt, lg_ns);
+            const uint8_t *mb = (FUSED && L.st) ? f.mat2 + (size_t)L.tso * bf_mat_bytes(K) : mat + (size_t)((!FUSED && g.matsel) ? L.tso : 0) * bf_mat_bytes(K);
 #pragma unroll
             for (int ch = 0; ch < NCH; ch++) {  // one copy per chunk: its two parity blocks are adjacent in the table
                 const int cs = ch % BF_NCS;
@@ -358,17 +425,25 @@ __global__ void __launch_bounds__(BF_THREADS, 1) stage_bf_kernel(StageGeom g, co
         uint32_t it = 0;
         for (long long tile; (tile = bf_tile(it)) < ntiles; it++) {
             const uint32_t buf = it & 1;
-            int tb, ts, to;
-            tile_coords_pow2(g, tile, lg_nbt, lg_ns, tb, ts, to);
-            const bool valid = tb * BF_COLS + c < g.ncols;
-            const uint4 *src = in + (col_off(g.ci, tb, c) + (long long)ts * g.is + (long long)to * g.io + (long long)par * g.ji);
-            const long long jstep = 2 * g.ji;
+            const BfLoc L = bf_locate<FUSED>(g, f, tile, lg_nbt, lg_ns);
+            const bool second = FUSED && L.st;  // second-stage tile of a fused axis: reads the ring
+            const bool valid = FUSED || L.tbi * BF_COLS + c < g.ncols;
+            const long long ji = second ? f.g2.ji : g.ji;
+            const uint4 *src = second
+                ? f.ring + ((long long)(L.grp % f.R) * BF_GROUP_ELEMS + col_off(f.g2.ci, L.tbi, c) + (long long)L.tsi * f.g2.is + (long long)par * ji)
+                : in + (col_off(g.ci, L.tbi, c) + (long long)L.tsi * g.is + (long long)L.toi * g.io + (long long)par * ji);
+            const long long jstep = 2 * ji;
+            if (FUSED) {  // the ring hand-shake (see BfFuse): data of this group written / the slot to be overwritten read
+                if (second) bf_wait_global(f.wr_done + L.grp, BF_WR_TARGET);
+                else if (L.grp >= f.R) bf_wait_global(f.rd_done + (L.grp - f.R), BF_RD_TARGET);
+                __syncwarp();
+            }
             // [ledger: a2 column exponent]
             // a2: column exponent = max of the 11-bit exponent fields (integer compare on the high words)
             uint32_t hmax = 0;
 #pragma unroll
             for (int jj = 0; jj < H; jj++) {
-                const uint4 v = valid ? __ldg(src + jj * jstep) : make_uint4(0, 0, 0, 0);
+                const uint4 v = valid ? bf_ld<FUSED>(src + jj * jstep) : make_uint4(0, 0, 0, 0);
                 hmax = max(hmax, max(v.y & 0x7FFFFFFFu, v.w & 0x7FFFFFFFu));
             }
             hmax = max(hmax, __shfl_xor_sync(0xFFFFFFFFu, hmax, 16));
@@ -379,7 +454,7 @@ __global__ void __launch_bounds__(BF_THREADS, 1) stage_bf_kernel(StageGeom g, co
             if (__any_sync(0xFFFFFFFFu, ef == 0)) {  // some column holds only zeros and subnormals: true leading bits
                 int tm = -100000;                   // (warp-uniform branch: the exchange below needs every lane)
                 for (int jj = 0; jj < H; jj++) {
-                    const uint4 v = valid ? __ldg(src + jj * jstep) : make_uint4(0, 0, 0, 0);
+                    const uint4 v = valid ? bf_ld<FUSED>(src + jj * jstep) : make_uint4(0, 0, 0, 0);
                     int T;
                     if (classify_top(((uint64_t)v.y << 32) | v.x, T) == CLS_FINITE) tm = max(tm, T);
                     if (classify_top(((uint64_t)v.w << 32) | v.z, T) == CLS_FINITE) tm = max(tm, T);
@@ -400,7 +475,7 @@ __global__ void __launch_bounds__(BF_THREADS, 1) stage_bf_kernel(StageGeom g, co
             for (int e0 = 0; e0 < H; e0 += BS) {
                 uint4 vv[BS];
 #pragma unroll
-                for (int x = 0; x < BS; x++) vv[x] = valid ? __ldg(src + (e0 + x) * jstep) : make_uint4(0, 0, 0, 0);
+                for (int x = 0; x < BS; x++) vv[x] = valid ? bf_ld<FUSED>(src + (e0 + x) * jstep) : make_uint4(0, 0, 0, 0);
 #pragma unroll
                 for (int x = 0; x < BS; x++) {
                     const int e = e0 + x;
@@ -434,7 +509,19 @@ __global__ void __launch_bounds__(BF_THREADS, 1) stage_bf_kernel(StageGeom g, co
             if (it >= 1) bf_wait_slack(&e_start[0], (it - 1) & 1);
             fence_async_smem();
             __syncwarp();
-            if (lane == 0) mbar_arrive(&a_full[0]);
+            if (second) {
+                // this warp's share of the ring slot (16 columns x 32 elements = 8 KB) has been consumed: drop the lines from L2
+                // without a write-back (Y' is dead until the slot is written again), 256 bytes per lane, then report the read
+                const int col = dw * 16 + (ji == 1 ? (lane >> 1) : 0), j0 = ji == 1 ? (lane & 1) * 16 : lane;
+                const uint4 *dl = f.ring + ((long long)(L.grp % f.R) * BF_GROUP_ELEMS + col_off(f.g2.ci, L.tbi, col) + (long long)L.tsi * f.g2.is + (long long)j0 * ji);
+                asm volatile("discard.global.L2 [%0], 128;" ::"l"(dl) : "memory");
+                asm volatile("discard.global.L2 [%0], 128;" ::"l"(dl + 8) : "memory");
+                __syncwarp();
+            }
+            if (lane == 0) {
+                mbar_arrive(&a_full[0]);
+                if (second) atomicAdd(f.rd_done + L.grp, 1u);
+            }
         }
     } else if (warp >= 12) {
         // [ledger: a12 store + addressing]
@@ -447,19 +534,29 @@ __global__ void __launch_bounds__(BF_THREADS, 1) stage_bf_kernel(StageGeom g, co
         const long long tstart_ = clock64();
 #endif
         int turn = qd;            // units to skip until the next one of this group (units go round-robin over the groups)
+        unsigned int wr_cnt = 0;  // fused axis: units of a first-stage tile this warp has stored and not yet counted
+        int wr_grp = 0;
         for (long long tile; (tile = bf_tile(it)) < ntiles; it++) {
             const uint32_t buf = it & 1;
-            int tb, ts, to;
-            tile_coords_pow2(g, tile, lg_nbt, lg_ns, tb, ts, to);
-            const bool valid = tb * BF_COLS + row < g.ncols;
-            uint4 *dstp = out + (col_off(g.co, tb, row) + (long long)ts * g.os + (long long)to * g.oo);
-            const uint4 *ct = ctab + (size_t)(g.matsel ? ts : 0) * K;
+            if (FUSED && wr_cnt) {  // first-stage stores of the previous tile: visible, then counted (before any wait of this tile)
+                __threadfence();
+                __syncwarp();
+                if (lane == 0) atomicAdd(f.wr_done + wr_grp, wr_cnt);
+                wr_cnt = 0;
+            }
+            const BfLoc L = bf_locate<FUSED>(g, f, tile, lg_nbt, lg_ns);
+            const bool second = FUSED && L.st;
+            const bool valid = FUSED || L.tbo * BF_COLS + row < g.ncols;
+            const long long ko = second ? f.g2.ko : g.ko;
+            uint4 *dstp = second ? out + (col_off(f.g2.co, L.tbo, row) + (long long)L.tso * f.g2.os + (long long)L.too * f.g2.oo)
+                          : (FUSED ? f.ring + (long long)(L.grp % f.R) * BF_GROUP_ELEMS : out) + (col_off(g.co, L.tbo, row) + (long long)L.tso * g.os + (long long)L.too * g.oo);
+            const uint4 *ct = second ? f.ctab2 + (size_t)L.tso * K : ctab + (size_t)((!FUSED && g.matsel) ? L.tso : 0) * K;
             { OZ_T0(); bf_wait_slack(&a_full[0], it & 1); OZ_T1(6); }  // the column exponents of this tile are published (s_T is double buffered: the
             const int Tmax = s_T[buf][row], flag = s_flag[buf][row];  // deconstruction runs at most one tile ahead)
             __syncwarp();
             if (lane == 0) mbar_arrive(&e_start[0]);
             const int gexp = 53 + 52 - Tmax;
-            const long long hko = (long long)H * g.ko;  // output k + H sits this far from output k
+            const long long hko = (long long)H * ko;  // output k + H sits this far from output k
 #pragma unroll 1
             for (int ch = 0; ch < NCH; ch++)
 #pragma unroll 1
@@ -487,7 +584,7 @@ __global__ void __launch_bounds__(BF_THREADS, 1) stage_bf_kernel(StageGeom g, co
                     nu++;
                     if (kp >= H || !valid) continue;
                     // [ledger: a12 store + addressing]
-                    uint4 *dk = dstp + (long long)kp * g.ko;
+                    uint4 *dk = dstp + (long long)kp * ko;
                     if (flag == 1) {  // the usual column: finite, not all zero
                         // a8 lift + a9 pack of the four outputs as one straight-line block (finish_fast); the rare outputs that
                         // need the two-sided correction, are tiny against the column scale or leave the normal range are redone
@@ -506,7 +603,13 @@ __global__ void __launch_bounds__(BF_THREADS, 1) stage_bf_kernel(StageGeom g, co
                         dk[0] = make_uint4(0, hi, 0, hi);
                         dk[hko] = make_uint4(0, hi, 0, hi);
                     }
+                    if (FUSED && !second) { wr_cnt++; wr_grp = L.grp; }
                 }
+        }
+        if (FUSED && wr_cnt) {
+            __threadfence();
+            __syncwarp();
+            if (lane == 0) atomicAdd(f.wr_done + wr_grp, wr_cnt);
         }
 #ifdef OZFFT_PIPE_TIMERS
         if (warp == 12 && lane == 0) { g_bf_dbg[blockIdx.x][5] = dbg_[5]; g_bf_dbg[blockIdx.x][6] = dbg_[6]; g_bf_dbg[blockIdx.x][7] = clock64() - tstart_; }
@@ -523,16 +626,17 @@ inline bool stage_bf_launch_k(const StageGeom &g, const void *in, void *out, con
                               long long nt, int sms, cudaStream_t st) {
     const long long pairs = (nt + 1) / 2;  // CTAs walk pairs of consecutive tiles (bf_tile)
     const unsigned grid = (unsigned)(pairs < sms ? pairs : sms);
-    stage_bf_kernel<K><<<grid, BF_THREADS, bf_smem_bytes<K>(), st>>>(g, (const uint4 *)in, (uint4 *)out, mat, (const uint4 *)ctab, (const uint4 *)pa, nt);
+    stage_bf_kernel<K, false><<<grid, BF_THREADS, bf_smem_bytes<K>(), st>>>(g, (const uint4 *)in, (uint4 *)out, mat, (const uint4 *)ctab, (const uint4 *)pa, nt, BfFuse{});
     return cudaGetLastError() == cudaSuccess;
 }
 
 inline bool stage_bf_prepare() {
-    cudaError_t e = cudaFuncSetAttribute(stage_bf_kernel<32>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bf_smem_bytes<32>());
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(stage_bf_kernel<16>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bf_smem_bytes<16>());
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(stage_bf_kernel<8>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bf_smem_bytes<8>());
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(stage_bf_kernel<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bf_smem_bytes<4>());
-    if (e == cudaSuccess) e = cudaFuncSetAttribute(stage_bf_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bf_smem_bytes<2>());
+    cudaError_t e = cudaFuncSetAttribute(stage_bf_kernel<32, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bf_smem_bytes<32>());
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(stage_bf_kernel<32, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bf_smem_bytes<32>());
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(stage_bf_kernel<16, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bf_smem_bytes<16>());
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(stage_bf_kernel<8, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bf_smem_bytes<8>());
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(stage_bf_kernel<4, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bf_smem_bytes<4>());
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(stage_bf_kernel<2, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bf_smem_bytes<2>());
     return e == cudaSuccess;
 }
 
@@ -552,6 +656,19 @@ inline bool stage_bf_launch(const StageGeom &g, const void *src, void *dst, cons
         case 2: return stage_bf_launch_k<2>(g, src, dst, mat, ctab, pa, nt, sms, st);
     }
     return false;
+}
+
+// both stages of one axis of length 1024 in one launch (BfFuse): g1 = first stage (output side = ring), f.g2 = second stage
+// (input side = ring).  The group counters are zeroed on the stream first.
+inline bool stage_bf_launch_fused(const StageGeom &g1, const BfFuse &f, const void *src, void *dst, const uint8_t *mat1, const void *ctab1,
+                                  const void *pa, int sms, cudaStream_t st) {
+    if (g1.K != 32 || f.g2.K != 32 || f.R <= f.Lg || f.Lg > f.G) return false;
+    if (cudaMemsetAsync(f.wr_done, 0, (size_t)f.G * 4, st) != cudaSuccess || cudaMemsetAsync(f.rd_done, 0, (size_t)f.G * 4, st) != cudaSuccess) return false;
+    const long long nt = 2LL * f.G * 32;
+    const long long pairs = nt / 2;
+    const unsigned grid = (unsigned)(pairs < sms ? pairs : sms);
+    stage_bf_kernel<32, true><<<grid, BF_THREADS, bf_smem_bytes<32>(), st>>>(g1, (const uint4 *)src, (uint4 *)dst, mat1, (const uint4 *)ctab1, (const uint4 *)pa, nt, f);
+    return cudaGetLastError() == cudaSuccess;
 }
 
 }  // namespace oz
