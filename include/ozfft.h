@@ -17,8 +17,11 @@
  * A plan must not execute concurrently on two streams (it owns workspace); different plans may be created and
  * executed from different host threads.  A destroyed or unknown handle is refused with OZFFT_EINVAL (the library
  * keeps a registry of live plans; it never dereferences a stale pointer).  Kernel selection: environment variable
- * OZFFT_VARIANT = bf (default: byte-fed tensor-core kernel), tc (residue-digit tensor-core kernel), simt, read at
- * plan creation.  No CPU fallback exists.
+ * OZFFT_VARIANT = bf (default: byte-fed tensor-core kernel), tc (residue-digit tensor-core kernel), simt, fp8 (kind::f8f6f4
+ * rung), garner / fp64sum (ablations), read at plan creation.  OZFFT_SCHEDULE = unfused makes the byte-fed kernel run
+ * every axis as two launches; by default an axis of length 1024 runs both stages in one launch with the intermediate
+ * array in an L2-resident ring.  Results are bit-identical for every variant but fp64sum and for
+ * both schedules.  No CPU fallback exists.
  */
 #ifndef OZFFT_H
 #define OZFFT_H

@@ -1,0 +1,77 @@
+"""GPU parity of the two schedules of the byte-fed kernel (Alg. 1 lines 7-8 at 220-241):
+fused -- both stages of an axis of length 1024 in one launch, Y' in an L2-resident ring -- and unfused (two launches per
+axis, OZFFT_SCHEDULE=unfused).  Both must equal the oracle bit for bit.  The shapes cover: the contiguous axis fused
+(ring [k2][pencil][j1]), a strided axis fused (ring [k2][j1][lane]), the strided axis that also takes the z permutation
+out (8 x 16 patch, p = 8 and p = 32), more groups than ring slots (slot reuse, both hand-shakes), a fused axis next to an
+unfusable one (inner length 2), and the batched 1-D plan."""
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+SHAPES = [((8, 64, 1024), 5, 4),     # z fused (4 groups), y two unfused stages with the patch (p = 32)
+          ((1024, 4, 128), 6, 4),    # x fused (strided, 4 groups)
+          ((2, 1024, 256), 7, 4),    # y fused AND un-permuting (patch, p = 8); z permuted (nz = 256)
+          ((8, 256, 1024), 8, 4),    # z fused with 16 groups > 14 ring slots
+          ((1024, 1024, 2), 9, 4)]   # x fused, y cannot be (inner length 2)
+
+
+def _bits(a):
+    return np.ascontiguousarray(a).view(np.uint64)
+
+
+@pytest.fixture(params=["fused", "unfused"])
+def schedule(request, monkeypatch):
+    monkeypatch.setenv("OZFFT_VARIANT", "bf")
+    monkeypatch.setenv("OZFFT_SCHEDULE", request.param)
+    return request.param
+
+
+@pytest.mark.parametrize("shape,seed,fused_launches", SHAPES)
+@pytest.mark.parametrize("sign", [-1, +1])
+def test_schedules_bit_exact_3d(O, schedule, shape, seed, fused_launches, sign):
+    import torch
+    from paper_2606_23698_b200 import inputs, ozfft
+    x = inputs.uniform_pm1(shape, seed)
+    plan = ozfft.Plan(*shape, sign=sign)
+    if schedule == "fused":
+        assert plan.num_launches == fused_launches
+    y = plan.exec(torch.from_numpy(x).cuda())
+    torch.cuda.synchronize()
+    got = y.cpu().numpy()
+    # a second execution of the same plan reuses the ring and the counters
+    y2 = plan.exec(torch.from_numpy(x).cuda())
+    torch.cuda.synchronize()
+    plan.destroy()
+    want, _ = O.fft3d(x, sign, route=0)
+    assert np.array_equal(_bits(got), _bits(want))
+    assert np.array_equal(_bits(y2.cpu().numpy()), _bits(want))
+
+
+def test_schedules_bit_exact_batched_1d(O, schedule):
+    import torch
+    from paper_2606_23698_b200 import inputs, ozfft
+    x = inputs.normal((2048, 1024), 2)
+    plan = ozfft.Plan.batched_1d(1024, 2048)
+    assert plan.num_launches == (1 if schedule == "fused" else 2)
+    got = plan.exec(torch.from_numpy(x).cuda()).cpu().numpy()
+    plan.destroy()
+    want, _ = O.fft1d(x, -1, route=0)
+    assert np.array_equal(_bits(got), _bits(want))
+
+
+def test_axis_hook_matches_fused_transform(schedule):
+    """ozfft_exec_axis runs every pass with natural-order intermediates; the one-call transform (fused axes, permuted z
+    between the z and y passes) must equal the composition of the three passes."""
+    import torch
+    from paper_2606_23698_b200 import inputs, ozfft
+    shape = (4, 1024, 1024)
+    x = torch.from_numpy(inputs.uniform_pm1(shape, 10)).cuda()
+    plan = ozfft.Plan(*shape)
+    cur = x
+    for axis in range(3):
+        cur = plan.exec_axis(axis, cur)
+    full = plan.exec(x)
+    torch.cuda.synchronize()
+    plan.destroy()
+    assert torch.equal(full.view(torch.float64), cur.view(torch.float64))
