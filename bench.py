@@ -98,14 +98,8 @@ def max_over_ranks(values, device="cpu"):
 
 
 def kernel_source_hash():
-    """sha256 over the kernel sources (csrc/*, include/*): ties a stored ncu figure to the code it was measured on"""
-    import glob
-    import hashlib
-    h = hashlib.sha256()
-    for f in sorted(glob.glob(os.path.join(ROOT, "paper_2606_23698_b200", "csrc", "*")) + glob.glob(os.path.join(ROOT, "include", "*.h"))):
-        h.update(os.path.basename(f).encode())
-        h.update(open(f, "rb").read())
-    return h.hexdigest()[:16]
+    from paper_2606_23698_b200 import ledger
+    return ledger.kernel_source_hash()
 
 
 def ncu_constants(size, variant):
@@ -119,7 +113,7 @@ def ncu_constants(size, variant):
     if db.get("source_hash") != kernel_source_hash():
         return None, f"stale: profiles/ncu_constants.json was captured on source hash {db.get('source_hash')}, the tree is {kernel_source_hash()}"
     e = db.get("entries", {}).get(f"{variant}:{size}")
-    return (e, db.get("command", "")) if e else (None, f"no ncu capture for variant {variant} at size {size}")
+    return (e, e.get("command", "")) if e else (None, f"no ncu capture for variant {variant} at size {size}")
 
 
 
@@ -307,14 +301,18 @@ def run_ours(args):
     if rank == 0:
         peak, peak_src = peaks()
         variant = os.environ.get("OZFFT_VARIANT", "bf")
+        schedule = os.environ.get("OZFFT_SCHEDULE", "fused") if variant == "bf" else "unfused"
+        stage_gemms = 3 * (2 if size > 32 else 1)  # per transform (Eq. 12: n_out = stage GEMMs x 2 N_tot)
+        n_out = 2 * stage_gemms * n_tot
         # algorithmic bytes = 32 B per element per AXIS PASS (16 read + 16 written) =
         # 96 N_tot per transform; a transform is `launches` stage launches of one kernel (two per axis when n > 32), so
-        # one launch accounts for 96 N_tot / launches algorithmic bytes.  The measured DRAM traffic of a launch is
-        # 32 N_tot (the intermediate array Y' crosses HBM: beta = 2, reported beside the fraction).
+        # one launch accounts for 96 N_tot / launches algorithmic bytes.  Fused schedule: one launch per axis, measured DRAM
+        # traffic 1.00 x 32 N_tot (beta = 1); unfused: two launches per axis, Y' crosses HBM (beta = 2).  beta is reported
+        # beside the fraction from the ncu capture recorded in profiles/ncu_constants.json.
         alg_bytes_launch = 96.0 * n_tot / launches
         launch_ms = ms_step / launches
         achieved = alg_bytes_launch / (launch_ms * 1e-3) / 1e9
-        ncu, ncu_note = ncu_constants(size, variant)
+        ncu, ncu_note = ncu_constants(size, variant if schedule != "unfused" or variant != "bf" else "bf-unfused")
         traffic = ncu["dram_bytes_per_launch"] if ncu else None
         tinst = ncu["thread_inst_per_output_eq"] if ncu else None
         line = {
@@ -323,14 +321,15 @@ def run_ours(args):
             "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "int32", "data": "synthetic",
             "config": {"workload": workload_name(size),
                        "parallelism": "replicas only" if world > 1 else "single GPU", "l2": "inputs_exceed_l2" if nbytes > (126 << 20) else "l2_resident",
-                       "variant": variant, "stage_launches_per_transform": launches},
+                       "variant": variant, "schedule": schedule, "stage_launches_per_transform": launches, "stage_gemms_per_transform": stage_gemms},
             "ms_per_transform": ms_step_max, "ms_per_transform_min": min(ms), "inverse_ms": inv_ms,
             "roundtrip_rel_err": roundtrip, "host_and_device_paths_bit_identical": same,
-            "hbm_roof": {"alg_bytes": 96.0 * n_tot if launches == 6 else alg_bytes_launch * launches / 2,
+            "hbm_roof": {"alg_bytes": 96.0 * n_tot,
                          "roof_ms_at_measured_peak": 96.0 * n_tot / (peak * 1e9) * 1e3, "frac_of_roof": (96.0 * n_tot / (peak * 1e9) * 1e3) / ms_step},
             "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
                          "traffic": traffic, "beta": (traffic / alg_bytes_launch if traffic else None),
-                         "kernel": {"bf": "stage_bf_kernel", "tc": "stage_tc_kernel", "simt": "stage_simt_kernel"}.get(variant, variant) + " (every launch of a transform is this kernel)",
+                         "kernel": {"bf": "stage_bf_kernel", "tc": "stage_tc_kernel", "simt": "stage_simt_kernel"}.get(variant, variant) + " (every launch of a transform is this kernel"
+                                   + ("; fused schedule: one launch per axis, both stages, Y' in an L2-resident ring)" if schedule == "fused" else ")"),
                          "peak_source": peak_src, "alg_bytes_per_launch": alg_bytes_launch, "launch_ms": launch_ms,
                          "ncu": ncu_note},
             "clocks": clocks,
@@ -342,10 +341,10 @@ def run_ours(args):
             # the SIMT side (PAPER.md:452 names integer issue as the wall): achieved = n_out x the ncu-measured thread
             # instructions per output-equivalent / step time; peak = 148 SM x 128 lanes x 1.965 GHz.
             # null when no ncu capture matches the current kernel sources.
-            "roofline_alu": ({"bound": "alu", "achieved": 2 * launches * n_tot * tinst / (ms_step * 1e-3) / 1e12,
+            "roofline_alu": ({"bound": "alu", "achieved": n_out * tinst / (ms_step * 1e-3) / 1e12,
                               "peak": 148 * 128 * 1.965e9 / 1e12, "unit": "T thread-inst/s",
-                              "frac": 2 * launches * n_tot * tinst / (ms_step * 1e-3) / (148 * 128 * 1.965e9),
-                              "n_out": 2 * launches * n_tot, "thread_inst_per_output_eq": tinst} if tinst else None),
+                              "frac": n_out * tinst / (ms_step * 1e-3) / (148 * 128 * 1.965e9),
+                              "n_out": n_out, "thread_inst_per_output_eq": tinst} if tinst else None),
             "context": {"cufft_z2z_ms": cufft_ms, "paper_projection_ms_B300": [63, 87], "paper_projection_ms_B200": [70, 96],
                         "paper_hbm_roof_ms": 12.9},
         }
@@ -406,14 +405,79 @@ def run_configs(args):
             cmed, _ = timed(cufft)
         except Exception:
             cmed = None
+        # variants other than the default: the same transform on the default kernel, compared on the device (the exact
+        # variants must be bit-identical; fp64sum, the naive fp64 Phase B of PAPER.md:340-345, shows its lost bits here)
+        same = diff = None
+        variant = os.environ.get("OZFFT_VARIANT", "bf")
+        if variant != "bf" or os.environ.get("OZFFT_SCHEDULE"):
+            keep = {k: os.environ.pop(k, None) for k in ("OZFFT_VARIANT", "OZFFT_SCHEDULE")}
+            ref_plan = ozfft.Plan(*shape) if kind == "3d" else ozfft.Plan.batched_1d(shape[1], shape[0])
+            for k, v in keep.items():
+                if v is not None:
+                    os.environ[k] = v
+            yref = ref_plan.exec(x)
+            torch.cuda.synchronize()
+            same = bool(torch.equal(y.view(torch.float64), yref.view(torch.float64)))
+            num = den = 0.0
+            fy, fr = y.view(-1), yref.view(-1)
+            for s0 in range(0, fy.numel(), 1 << 26):
+                num += float(((fy[s0:s0 + (1 << 26)] - fr[s0:s0 + (1 << 26)]).abs() ** 2).sum())
+                den += float((fr[s0:s0 + (1 << 26)].abs() ** 2).sum())
+            diff = math.sqrt(num / den)
+            ref_plan.destroy()
+            del yref
         roof_ms = 32.0 * x.numel() * passes / (hbm * 1e9) * 1e3
-        print(json.dumps({"config": name, "variant": os.environ.get("OZFFT_VARIANT", "bf"), "shape": list(shape), "input": dist_name,
+        print(json.dumps({"config": name, "variant": variant, "schedule": os.environ.get("OZFFT_SCHEDULE", "fused" if variant == "bf" else "unfused"),
+                          "bit_identical_to_default_kernel": same, "normwise_diff_vs_default_kernel": diff, "shape": list(shape), "input": dist_name,
                           "seed": seed, "launches": plan.num_launches, "ms_median": med, "ms_best": best,
                           "gflops_5NlogN": flop / (med * 1e-3) / 1e9, "hbm_roof_ms": roof_ms, "frac_of_hbm_roof": roof_ms / med,
                           "cufft_z2z_ms": cmed}), flush=True)
         plan.destroy()
         del x, y, h
         torch.cuda.empty_cache()
+
+
+def run_pipe_timers(args):
+    """--pipe-timers: where the byte-fed kernel's roles wait.  Builds and loads the measuring library (build.py --timers:
+    clock64 stamps around every mbarrier wait), runs one transform per axis pass and prints, per launch, the cycles per
+    tile each role spent waiting (mean over the CTAs).  Not a timed run: the stamps cost issue slots."""
+    import ctypes
+    import numpy as np
+    import torch
+    from paper_2606_23698_b200 import build as b, ozfft
+    ozfft._SO = b.build(timers=True)
+    L = ozfft.lib()
+    size = args.size
+    x = torch.randn(size, size, size, dtype=torch.complex128, device="cuda")
+    plan = ozfft.Plan(size, size, size)
+    buf = (ctypes.c_ulonglong * (160 * 12))()
+    y = plan.exec(x)
+    torch.cuda.synchronize()
+    sms = torch.cuda.get_device_properties(0).multi_processor_count
+    names = ["z", "y", "x"]
+    for axis in range(3):
+        # the stamps are those of the LAST launch: the axis hook (unfused, natural order) ends with the axis' second stage
+        plan.exec_axis(axis, x, y)
+        torch.cuda.synchronize()
+        assert L.ozfft_debug_timers(buf) == 160
+        a = np.frombuffer(buf, dtype=np.uint64).reshape(160, 12)[:sms].astype(np.float64)
+        t = a[:, 4].mean()
+        print(json.dumps({"launch": f"{names[axis]} pass, second stage (axis hook, unfused, natural order)", "tiles_per_cta": t,
+                          "issuer_wait_a_full": a[:, 0].mean() / t, "issuer_wait_b_full": a[:, 1].mean() / t, "issuer_wait_pa_empty": a[:, 2].mean() / t,
+                          "issuer_total": a[:, 3].mean() / t, "epilogue_wait_pa_full": a[:, 5].mean() / t, "epilogue_wait_a_full": a[:, 6].mean() / t,
+                          "epilogue_total": a[:, 7].mean() / t, "decon_wait_ring": a[:, 8].mean() / t, "decon_wait_a_empty_e_start": a[:, 9].mean() / t,
+                          "decon_total": a[:, 10].mean() / t, "unit": "SM cycles per tile"}))
+    plan.exec(x, y)
+    torch.cuda.synchronize()
+    assert L.ozfft_debug_timers(buf) == 160
+    a = np.frombuffer(buf, dtype=np.uint64).reshape(160, 12)[:sms].astype(np.float64)
+    t = a[:, 4].mean()
+    print(json.dumps({"launch": "x pass of the one-call transform (" + os.environ.get("OZFFT_SCHEDULE", "fused") + " schedule; a fused launch holds both stages)",
+                      "tiles_per_cta": t, "issuer_wait_a_full": a[:, 0].mean() / t, "issuer_wait_b_full": a[:, 1].mean() / t,
+                      "issuer_wait_pa_empty": a[:, 2].mean() / t, "issuer_total": a[:, 3].mean() / t, "epilogue_wait_pa_full": a[:, 5].mean() / t,
+                      "epilogue_wait_a_full": a[:, 6].mean() / t, "epilogue_total": a[:, 7].mean() / t, "decon_wait_ring": a[:, 8].mean() / t,
+                      "decon_wait_a_empty_e_start": a[:, 9].mean() / t, "decon_total": a[:, 10].mean() / t, "unit": "SM cycles per tile"}))
+    plan.destroy()
 
 
 def main():
@@ -425,6 +489,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg (profiling runs)")
     ap.add_argument("--configs", action="store_true", help="time all five BASELINE.json configs (one JSON line each) instead of the contract line")
+    ap.add_argument("--pipe-timers", action="store_true", help="per-role wait cycles of the byte-fed kernel (measuring build; not a timed run)")
     ap.add_argument("--dry-run", action="store_true", help="launch plumbing only (gloo, no GPU work): used by the CPU tests")
     args = ap.parse_args()
     if args.gpus > 1 and "WORLD_SIZE" not in os.environ:
@@ -436,7 +501,9 @@ def main():
         cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={args.gpus}", "--master-addr", "127.0.0.1",
                "--master-port", str(port), os.path.abspath(__file__)] + sys.argv[1:]
         raise SystemExit(subprocess.call(cmd))
-    if args.configs:
+    if args.pipe_timers:
+        run_pipe_timers(args)
+    elif args.configs:
         run_configs(args)
     elif args.impl == "reference":
         run_reference(args)

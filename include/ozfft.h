@@ -87,6 +87,14 @@ int ozfft_probe_cp(int kbytes, const void *dA, void *dD, void *stream);
  * Synchronises `stream`.  Device pointers. */
 int ozfft_probe_crt(int n, const void *d_residues, void *d_out, int variant, void *stream);
 
+/* Pipeline timers of the byte-fed stage kernel (measuring build only: paper_2606_23698_b200/build.py --timers compiles with
+ * -DOZFFT_PIPE_TIMERS; the product build returns 0 and writes nothing).  h receives 160 x 12 uint64 (HOST pointer), one row per
+ * CTA of the LAST launch, in SM clock cycles summed over the CTA's tiles: [0] issuer waiting for the data operand (a_full),
+ * [1] for matrix planes (b_full), [2] for the Phase-A result slots (pa_empty), [3] issuer loop total, [4] tiles of the CTA,
+ * [5] epilogue warp 12 waiting for Phase-A results, [6] for the column exponents, [7] its loop total, [8] deconstruction
+ * warp 4 waiting on the fused-axis ring counters, [9] on a_empty / e_start, [10] its loop total.  Returns the row count. */
+int ozfft_debug_timers(unsigned long long *h);
+
 #ifdef __cplusplus
 }
 #endif

@@ -17,18 +17,27 @@ def _deps():
     return sources() + glob.glob(os.path.join(CSRC, "*.cuh")) + glob.glob(os.path.join(_ROOT, "include", "*.h"))
 
 
-def build(force=False, verbose=False):
-    if not force and os.path.exists(SO) and os.path.getmtime(SO) >= max(os.path.getmtime(f) for f in _deps()):
-        return SO
+SO_TIMERS = os.path.join(_HERE, "libozfft_timers.so")
+
+
+def build(force=False, verbose=False, timers=False):
+    """timers=True builds libozfft_timers.so: the same library with -DOZFFT_PIPE_TIMERS (clock64 stamps around every
+    mbarrier wait of the byte-fed kernel's issuer and of one epilogue warp, read back by ozfft_debug_timers; a measuring
+    build for `bench.py --pipe-timers`, never the one that is timed)."""
+    so = SO_TIMERS if timers else SO
+    if not force and os.path.exists(so) and os.path.getmtime(so) >= max(os.path.getmtime(f) for f in _deps()):
+        return so
     cmd = ["nvcc", "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
            "-Xcompiler", "-fPIC", "-shared", "-I", os.path.join(_ROOT, "include"), "-I", CSRC,
-           "-o", SO] + sources() + ["-lcudart"]
+           "-o", so] + sources() + ["-lcudart"]
+    if timers:
+        cmd.insert(1, "-DOZFFT_PIPE_TIMERS")
     if verbose:
         cmd.insert(1, "-Xptxas=-v")
     subprocess.check_call(cmd)
-    return SO
+    return so
 
 
 if __name__ == "__main__":
     import sys
-    print(build(force=True, verbose="-v" in sys.argv))
+    print(build(force=True, verbose="-v" in sys.argv, timers="--timers" in sys.argv))

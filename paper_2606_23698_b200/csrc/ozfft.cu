@@ -304,10 +304,13 @@ bool add_axis(ozfft_plan_s *p, const AxisDesc &a, int axis, MatMap &mats, std::v
         if (unperm) f.g2.co = g1.co;  // the group's 128 columns are the 8 x 16 patch: the second stage stores them at their natural places
         sf.g.os = 0; sf.g.oo = 0; sf.g.ko = 4096;
         f.g2.is = 4096; f.g2.io = 0;
-        if (a.contiguous) {  // first-stage tile = 4 pencils x 32 j1 -> ring [k2][pencil][j1]; second-stage column = pencil
-            sf.g.co = StageGeom::ColMap{0, 0, 127, 7, 128, 0, 1, 0};
-            f.g2.ci = StageGeom::ColMap{0, 0, 127, 7, 0, 0, 32, 0};
-            f.g2.ji = 1;
+        if (a.contiguous) {
+            // first-stage tile = 4 pencils x 32 j1; second-stage column = pencil.  Ring [k2][j1][pencil]: the second stage's loads
+            // are coalesced across its columns like on the strided axes (its latency-bound side); the first stage pays with
+            // 16-byte stores 2 KB apart, which stay in L2
+            sf.g.co = StageGeom::ColMap{0, 0, 31, 5, 4, 0, 128, 1};
+            f.g2.ci = StageGeom::ColMap{0, 0, 127, 7, 0, 0, 1, 0};
+            f.g2.ji = 128;
             f.G = (int)(cols / 128);
             f.lg_nbt = 30;
             f.s1_mulb = 32; f.s1_tlb = 1; f.s1_tls = 0; f.r1_tlb = 1; f.r1_tls = 0;
@@ -362,10 +365,10 @@ ozfft_plan_s *make_plan(int nx, int ny, int nz, int sign, bool batched1d) {
     {   // schedule of the byte-fed kernel: axes of length 1024 run both stages in one launch unless OZFFT_SCHEDULE=unfused
         const char *sch = getenv("OZFFT_SCHEDULE");
         p->fuse = !(sch && !strcmp(sch, "unfused"));
-        // lag 8 groups, ring 14 slots = 28 MB (measured at 1024^3: lag 3 / 4 / 6 / 8 / 12 -> 191 / 144 / 131 / 130 / 132 ms: below ~6 the
+        // lag 8 groups, ring 16 slots = 32 MB (a power of two: the slot index is a mask; measured at 1024^3: lag 3 / 4 / 6 / 8 / 12 -> 191 / 144 / 131 / 130 / 132 ms: below ~6 the
         // second-stage tiles catch up with the first-stage tiles still in flight on the 148 SMs and wait)
         p->fuse_lag = 8;
-        p->ring_slots = 14;
+        p->ring_slots = 16;
     }
     p->pipelined = false;
     p->s_in = p->s_out = nullptr;
@@ -388,8 +391,10 @@ ozfft_plan_s *make_plan(int nx, int ny, int nz, int sign, bool batched1d) {
         ok = ok && add_axis(p, AxisDesc{true, nx, nz, 1}, 0, mats, p->stages, false, 0, p->fuse);
         if (ok && !p->stages.empty() && p->stages[0].fused) ok = add_axis(p, AxisDesc{true, nx, nz, 1}, 0, mats, p->stages_nat);
     } else {
-        // byte-fed kernel, nz >= 256: the z pass leaves its output permuted along z and the first y stage undoes it (stage.cuh)
-        const bool perm = p->variant == 2 && nz >= 256;
+        // byte-fed kernel, nz = 1024: the z pass leaves its output permuted along z and the first y stage undoes it (stage.cuh).
+        // Measured at nz = 512: the patch costs the y stage 0.5 ms and the z pass gains nothing (it is bound by its lane-per-pencil
+        // loads there, not by the partial sectors), so shorter z axes keep the natural order.
+        const bool perm = p->variant == 2 && nz == 1024;
         ok = ok && add_axis(p, AxisDesc{true, (long long)nx * ny, nz, 1}, 0, mats, p->stages, perm, 0, p->fuse);
         ok = ok && add_axis(p, AxisDesc{false, nx, ny, nz}, 1, mats, p->stages, false, perm ? nz / 32 : 0, p->fuse);
         ok = ok && add_axis(p, AxisDesc{false, 1, nx, (long long)ny * nz}, 2, mats, p->stages, false, 0, p->fuse);
@@ -678,9 +683,14 @@ size_t ozfft_debug_bf_tables(int K, int fusedN, int sign, void *h_B, void *h_C, 
     return B.size();
 }
 
+int ozfft_debug_timers(unsigned long long *h) {
 #ifdef OZFFT_PIPE_TIMERS
-void ozfft_debug_timers(unsigned long long *h) { cudaMemcpyFromSymbol(h, g_bf_dbg, sizeof(g_bf_dbg)); }
+    return cudaMemcpyFromSymbol(h, g_bf_dbg, sizeof(g_bf_dbg)) == cudaSuccess ? 160 : 0;
+#else
+    (void)h;
+    return 0;
 #endif
+}
 
 uint64_t ozfft_twiddle_checksum(void) { return twiddle_fnv(twiddles()); }
 

@@ -34,9 +34,14 @@ struct StageGeom {
     struct ColMap { int t_sh, t_mask, c_mask, c_sh; long long t_hi, t_lo, c_lo, c_hi; } ci, co;
 };
 
-__device__ __forceinline__ long long col_off(const StageGeom::ColMap &m, int tb, int c) {
-    return (long long)(tb >> m.t_sh) * m.t_hi + (long long)(tb & m.t_mask) * m.t_lo + (long long)(c & m.c_mask) * m.c_lo + (long long)(c >> m.c_sh) * m.c_hi;
+// the column part does not change from tile to tile (a thread keeps it), the tile part is the same for a whole warp
+__device__ __forceinline__ long long col_part(const StageGeom::ColMap &m, int c) {
+    return (long long)(c & m.c_mask) * m.c_lo + (long long)(c >> m.c_sh) * m.c_hi;
 }
+__device__ __forceinline__ long long tile_part(const StageGeom::ColMap &m, int tb) {
+    return (long long)(tb >> m.t_sh) * m.t_hi + (long long)(tb & m.t_mask) * m.t_lo;
+}
+__device__ __forceinline__ long long col_off(const StageGeom::ColMap &m, int tb, int c) { return tile_part(m, tb) + col_part(m, c); }
 
 // the same with nbt = 2^lg_nbt and ns = 2^lg_ns (every supported size is a power of two): shifts, no division
 __device__ __forceinline__ void tile_coords_pow2(const StageGeom &g, long long t, int lg_nbt, int lg_ns, int &b, int &s, int &o) {

@@ -142,7 +142,7 @@ template <int K> __host__ __device__ constexpr size_t bf_smem_bytes() {
 }
 
 #ifdef OZFFT_PIPE_TIMERS
-__device__ unsigned long long g_bf_dbg[160][8];
+__device__ unsigned long long g_bf_dbg[160][12];  // per CTA: see ozfft_debug_timers (include/ozfft.h)
 #define OZ_T0() const long long t0_ = clock64()
 #define OZ_T1(i) dbg_[i] += clock64() - t0_
 #else
@@ -200,7 +200,7 @@ struct BfFuse {
     const uint4 *ctab2;
     uint4 *ring;                   // R slots x 131072 elements
     unsigned int *wr_done, *rd_done;  // per group: first-stage (warp, unit) stores done; second-stage warps done reading
-    int G, Lg, R;                  // groups, lag, ring slots (R > Lg)
+    int G, Lg, R;                  // groups, lag, ring slots (R > Lg, a power of two)
     int lg_nbt;                    // group = (go << lg_nbt) | gb
     int s1_mulb, s1_tlb, s1_tls;   // first-stage input tile: tb = gb * s1_mulb + tl * s1_tlb, ts = tl * s1_tls, to = go
     int r1_tlb, r1_tls;            // first-stage output (ring) tile: tb = tl * r1_tlb, ts = tl * r1_tls
@@ -359,9 +359,13 @@ __global__ void __launch_bounds__(BF_THREADS, 1) stage_bf_kernel(StageGeom g, co
                 tc_commit(&pa_full[gg ? g1 : g0]);
             }
         };
+        constexpr int UNR = NCH < BF_NCS ? NCH : BF_NCS;  // unrolled once around the matrix ring (code size: the instruction cache)
         for (; bf_tile(it) < ntiles; it++) {
+#pragma unroll 1
+            for (int c4 = 0; c4 < NCH; c4 += UNR)
 #pragma unroll
-            for (int ch = 0; ch < NCH; ch++) {
+            for (int u = 0; u < UNR; u++) {
+                const int ch = c4 + u;
                 const uint32_t g0 = gc, g1 = gc + 1 == BF_NG ? 0 : gc + 1;
                 if (pend) wait_pa();
                 if (ch == 0) {  // tile boundary: Phase A of the previous tile's last chunk goes out before the wait for the new operand
@@ -372,7 +376,7 @@ __global__ void __launch_bounds__(BF_THREADS, 1) stage_bf_kernel(StageGeom g, co
                     }
                     { OZ_T0(); bf_wait(&a_full[0], it & 1); OZ_T1(0); }
                 }
-                { OZ_T0(); bf_wait(&b_full[ch % BF_NCS], (UPT * it + ch / BF_NCS) & 1); OZ_T1(1); }
+                { OZ_T0(); bf_wait(&b_full[u], (UPT * it + ch / BF_NCS) & 1); OZ_T1(1); }
                 tc_fence_after();
                 if (elect_one()) {
                     const uint32_t tz = tzero();
@@ -392,7 +396,7 @@ __global__ void __launch_bounds__(BF_THREADS, 1) stage_bf_kernel(StageGeom g, co
                     }
 #pragma unroll
                     for (int par = 0; par < 2; par++) {
-                        const uint64_t bd = bdz + (uint64_t)((((ch % BF_NCS) * 2 + par) * SB) >> 4);
+                        const uint64_t bd = bdz + (uint64_t)(((u * 2 + par) * SB) >> 4);
 #pragma unroll
                         for (int P = 0; P < 2; P++)  // P = 0: re rows [XR ; NXI] (planes 1, 2), P = 1: im rows [XI ; XR] (planes 0, 1)
 #pragma unroll
@@ -400,7 +404,7 @@ __global__ void __launch_bounds__(BF_THREADS, 1) stage_bf_kernel(StageGeom g, co
                                 mma_i8_ts(tz + (BF_TD + P * 96 + par * 48), tz + (BF_TA + par * ACOLS + ((1 - P) * NCK + 2 * s) * 4),
                                           bd + (uint64_t)((s * 2 * BF_N * 16) >> 4), idesc_st, s > 0);
                     }
-                    tc_commit(&b_empty[ch % BF_NCS]);
+                    tc_commit(&b_empty[u]);
                 }
                 __syncwarp();
                 if (pend) gc = g1 + 1 == BF_NG ? 0 : g1 + 1;
@@ -415,14 +419,21 @@ __global__ void __launch_bounds__(BF_THREADS, 1) stage_bf_kernel(StageGeom g, co
             __syncwarp();
         }
 #ifdef OZFFT_PIPE_TIMERS
-        if (lane == 0) { dbg_[3] = clock64() - tstart_; dbg_[4] = it; for (int i = 0; i < 8; i++) g_bf_dbg[blockIdx.x][i] = dbg_[i]; }
+        if (lane == 0) { dbg_[3] = clock64() - tstart_; dbg_[4] = it; for (int i = 0; i < 5; i++) g_bf_dbg[blockIdx.x][i] = dbg_[i]; }
 #endif
     } else if (warp >= 4 && warp < 12) {
         // [ledger: a1 load + addressing]
         // ------------------------------------------------ deconstruction: thread = (column, parity of j)
         const int dw = warp - 4, par = lane >> 4, c = dw * 16 + (lane & 15);
         constexpr int BS = H < 8 ? H : 8;  // elements loaded together (memory-level parallelism)
+        // this thread's column offset: kept across tiles in the two-launch kernel (every per-tile instruction counts at this
+        // utilisation: -13 % at 512^3); recomputed per tile in the fused kernel, where two more 64-bit values would spill
+        const long long cin1 = FUSED ? 0 : col_part(g.ci, c);
         uint32_t it = 0;
+#ifdef OZFFT_PIPE_TIMERS
+        long long dbg_[12] = {0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0};
+        const long long tstart_ = clock64();
+#endif
         for (long long tile; (tile = bf_tile(it)) < ntiles; it++) {
             const uint32_t buf = it & 1;
             const BfLoc L = bf_locate<FUSED>(g, f, tile, lg_nbt, lg_ns);
@@ -430,12 +441,14 @@ __global__ void __launch_bounds__(BF_THREADS, 1) stage_bf_kernel(StageGeom g, co
             const bool valid = FUSED || L.tbi * BF_COLS + c < g.ncols;
             const long long ji = second ? f.g2.ji : g.ji;
             const uint4 *src = second
-                ? f.ring + ((long long)(L.grp % f.R) * BF_GROUP_ELEMS + col_off(f.g2.ci, L.tbi, c) + (long long)L.tsi * f.g2.is + (long long)par * ji)
-                : in + (col_off(g.ci, L.tbi, c) + (long long)L.tsi * g.is + (long long)L.toi * g.io + (long long)par * ji);
+                ? f.ring + ((long long)(L.grp & (f.R - 1)) * BF_GROUP_ELEMS + col_off(f.g2.ci, L.tbi, c) + (long long)L.tsi * f.g2.is + (long long)par * ji)
+                : in + (tile_part(g.ci, L.tbi) + (FUSED ? col_part(g.ci, c) : cin1) + (long long)L.tsi * g.is + (long long)L.toi * g.io + (long long)par * ji);
             const long long jstep = 2 * ji;
             if (FUSED) {  // the ring hand-shake (see BfFuse): data of this group written / the slot to be overwritten read
+                OZ_T0();
                 if (second) bf_wait_global(f.wr_done + L.grp, BF_WR_TARGET);
                 else if (L.grp >= f.R) bf_wait_global(f.rd_done + (L.grp - f.R), BF_RD_TARGET);
+                OZ_T1(8);
                 __syncwarp();
             }
             // [ledger: a2 column exponent]
@@ -464,7 +477,7 @@ __global__ void __launch_bounds__(BF_THREADS, 1) stage_bf_kernel(StageGeom g, co
             }
             // [ledger: a3 deconstruction: quantise, offset, byte planes]
             // the previous tile's operand must have been copied to TMEM before the shared copy is overwritten
-            if (it >= 1) bf_wait_slack(&a_empty[0], (it - 1) & 1);
+            if (it >= 1) { OZ_T0(); bf_wait_slack(&a_empty[0], (it - 1) & 1); OZ_T1(9); }
             if (par == 0) { s_T[buf][c] = Tmax; s_flag[buf][c] = flag; }
             // a3: quantise, offset by 2^53, split into bytes; planes XI (0), XR (1), NXI (2)
             uint32_t wr[NW + 2], wi[NW + 2], wn[NW + 2];
@@ -506,14 +519,14 @@ __global__ void __launch_bounds__(BF_THREADS, 1) stage_bf_kernel(StageGeom g, co
                 }
             // every epilogue warp must have observed the a_full phase of tile it-1 (and read its exponents) before
             // this tile's phase may complete: a waiter that falls two phases behind would wait forever
-            if (it >= 1) bf_wait_slack(&e_start[0], (it - 1) & 1);
+            if (it >= 1) { OZ_T0(); bf_wait_slack(&e_start[0], (it - 1) & 1); OZ_T1(9); }
             fence_async_smem();
             __syncwarp();
             if (second) {
                 // this warp's share of the ring slot (16 columns x 32 elements = 8 KB) has been consumed: drop the lines from L2
                 // without a write-back (Y' is dead until the slot is written again), 256 bytes per lane, then report the read
                 const int col = dw * 16 + (ji == 1 ? (lane >> 1) : 0), j0 = ji == 1 ? (lane & 1) * 16 : lane;
-                const uint4 *dl = f.ring + ((long long)(L.grp % f.R) * BF_GROUP_ELEMS + col_off(f.g2.ci, L.tbi, col) + (long long)L.tsi * f.g2.is + (long long)j0 * ji);
+                const uint4 *dl = f.ring + ((long long)(L.grp & (f.R - 1)) * BF_GROUP_ELEMS + col_off(f.g2.ci, L.tbi, col) + (long long)L.tsi * f.g2.is + (long long)j0 * ji);
                 asm volatile("discard.global.L2 [%0], 128;" ::"l"(dl) : "memory");
                 asm volatile("discard.global.L2 [%0], 128;" ::"l"(dl + 8) : "memory");
                 __syncwarp();
@@ -523,6 +536,9 @@ __global__ void __launch_bounds__(BF_THREADS, 1) stage_bf_kernel(StageGeom g, co
                 if (second) atomicAdd(f.rd_done + L.grp, 1u);
             }
         }
+#ifdef OZFFT_PIPE_TIMERS
+        if (warp == 4 && lane == 0) { g_bf_dbg[blockIdx.x][8] = dbg_[8]; g_bf_dbg[blockIdx.x][9] = dbg_[9]; g_bf_dbg[blockIdx.x][10] = clock64() - tstart_; }
+#endif
     } else if (warp >= 12) {
         // [ledger: a12 store + addressing]
         // ------------------------------------------------ epilogue: thread = data column (TMEM lane), both parts
@@ -534,6 +550,7 @@ __global__ void __launch_bounds__(BF_THREADS, 1) stage_bf_kernel(StageGeom g, co
         const long long tstart_ = clock64();
 #endif
         int turn = qd;            // units to skip until the next one of this group (units go round-robin over the groups)
+        const long long cout1 = FUSED ? 0 : col_part(g.co, row);
         unsigned int wr_cnt = 0;  // fused axis: units of a first-stage tile this warp has stored and not yet counted
         int wr_grp = 0;
         for (long long tile; (tile = bf_tile(it)) < ntiles; it++) {
@@ -549,7 +566,7 @@ __global__ void __launch_bounds__(BF_THREADS, 1) stage_bf_kernel(StageGeom g, co
             const bool valid = FUSED || L.tbo * BF_COLS + row < g.ncols;
             const long long ko = second ? f.g2.ko : g.ko;
             uint4 *dstp = second ? out + (col_off(f.g2.co, L.tbo, row) + (long long)L.tso * f.g2.os + (long long)L.too * f.g2.oo)
-                          : (FUSED ? f.ring + (long long)(L.grp % f.R) * BF_GROUP_ELEMS : out) + (col_off(g.co, L.tbo, row) + (long long)L.tso * g.os + (long long)L.too * g.oo);
+                          : (FUSED ? f.ring + (long long)(L.grp & (f.R - 1)) * BF_GROUP_ELEMS : out) + (tile_part(g.co, L.tbo) + (FUSED ? col_part(g.co, row) : cout1) + (long long)L.tso * g.os + (long long)L.too * g.oo);
             const uint4 *ct = second ? f.ctab2 + (size_t)L.tso * K : ctab + (size_t)((!FUSED && g.matsel) ? L.tso : 0) * K;
             { OZ_T0(); bf_wait_slack(&a_full[0], it & 1); OZ_T1(6); }  // the column exponents of this tile are published (s_T is double buffered: the
             const int Tmax = s_T[buf][row], flag = s_flag[buf][row];  // deconstruction runs at most one tile ahead)
@@ -662,7 +679,7 @@ inline bool stage_bf_launch(const StageGeom &g, const void *src, void *dst, cons
 // (input side = ring).  The group counters are zeroed on the stream first.
 inline bool stage_bf_launch_fused(const StageGeom &g1, const BfFuse &f, const void *src, void *dst, const uint8_t *mat1, const void *ctab1,
                                   const void *pa, int sms, cudaStream_t st) {
-    if (g1.K != 32 || f.g2.K != 32 || f.R <= f.Lg || f.Lg > f.G) return false;
+    if (g1.K != 32 || f.g2.K != 32 || f.R <= f.Lg || (f.R & (f.R - 1)) || f.Lg > f.G) return false;
     if (cudaMemsetAsync(f.wr_done, 0, (size_t)f.G * 4, st) != cudaSuccess || cudaMemsetAsync(f.rd_done, 0, (size_t)f.G * 4, st) != cudaSuccess) return false;
     const long long nt = 2LL * f.G * 32;
     const long long pairs = nt / 2;

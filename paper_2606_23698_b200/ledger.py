@@ -1,6 +1,7 @@
 """Epilogue instruction ledger by term (PAPER.md:437-445 table, 558 eps_mix, 876, 890).
 
   python -m paper_2606_23698_b200.ledger REPORT.ncu-rep --n-out N [--launch I] [--md OUT.md] [--lines OUT.csv]
+  python -m paper_2606_23698_b200.ledger REPORT.ncu-rep --summary   # key raw metrics of every launch in the report
   python -m paper_2606_23698_b200.ledger --static            # SASS opcode histogram of the built library
 
 REPORT is one `ncu --set full --import-source on` capture of ONE stage-kernel launch (the recipe in
@@ -207,6 +208,81 @@ def static_histogram(so):
     return "\n".join(o)
 
 
+SUMMARY_KEYS = [
+    "gpu__time_duration.sum", "dram__bytes_read.sum", "dram__bytes_write.sum", "lts__t_sector_hit_rate.pct",
+    "smsp__inst_executed.sum", "smsp__thread_inst_executed.sum", "smsp__issue_active.avg.pct_of_peak_sustained_active",
+    "sm__warps_active.avg.pct_of_peak_sustained_active", "sm__pipe_tensor_cycles_active.avg.pct_of_peak_sustained_active",
+    "sm__inst_executed_pipe_alu.avg.pct_of_peak_sustained_active", "sm__inst_executed_pipe_fma.avg.pct_of_peak_sustained_active",
+    "sm__inst_executed_pipe_lsu.avg.pct_of_peak_sustained_active", "l1tex__data_bank_conflicts_pipe_lsu_mem_shared.sum",
+    "launch__registers_per_thread", "sm__cycles_elapsed.avg"]
+STALLS = ["long_scoreboard", "wait", "barrier", "not_selected", "math_pipe_throttle", "branch_resolving", "short_scoreboard",
+          "dispatch_stall", "no_instruction", "mio_throttle", "lg_throttle", "sleeping"]
+
+
+def summary(report):
+    """key raw metrics of EVERY launch in the report, one column per launch (markdown)"""
+    r = subprocess.run(["ncu", "-i", report, "--page", "raw", "--csv"], capture_output=True, text=True)
+    if r.returncode != 0:
+        raise SystemExit("ncu failed: " + r.stderr[-2000:])
+    rows = list(csv.reader(io.StringIO(r.stdout)))
+    hdr, units, launches = rows[0], rows[1], rows[2:]
+    o = ["| metric | unit | " + " | ".join(f"launch {i}" for i in range(len(launches))) + " |", "|---|---|" + "---|" * len(launches)]
+    o.append("| kernel | | " + " | ".join(re.sub(r"\(.*", "", l[hdr.index("Kernel Name")])[-40:] + " grid " + l[hdr.index("Grid Size")] for l in launches) + " |")
+    for k in SUMMARY_KEYS:
+        if k in hdr:
+            i = hdr.index(k)
+            o.append(f"| {k} | {units[i]} | " + " | ".join(l[i] for l in launches) + " |")
+    for st in STALLS:
+        k = f"smsp__average_warps_issue_stalled_{st}_per_issue_active.ratio"
+        if k in hdr:
+            i = hdr.index(k)
+            o.append(f"| stall {st} (warps per issue) | | " + " | ".join(f"{float(l[i]):.2f}" for l in launches) + " |")
+    return "\n".join(o)
+
+
+def kernel_source_hash():
+    """sha256 over the kernel sources (csrc/*, include/*.h): ties a stored ncu figure to the code it was measured on"""
+    import hashlib
+    h = hashlib.sha256()
+    root = os.path.dirname(_HERE)
+    for f in sorted(glob.glob(os.path.join(CSRC, "*")) + glob.glob(os.path.join(root, "include", "*.h"))):
+        h.update(os.path.basename(f).encode())
+        h.update(open(f, "rb").read())
+    return h.hexdigest()[:16]
+
+
+def constants(report, key, n_out, out_json, command):
+    """profiles/ncu_constants.json entry `key` (e.g. "bf:1024") from a report that holds ALL stage launches of one transform:
+    DRAM bytes per launch (mean), thread instructions per output-equivalent (sum over the launches / n_out)."""
+    import json
+    r = subprocess.run(["ncu", "-i", report, "--page", "raw", "--csv"], capture_output=True, text=True)
+    if r.returncode != 0:
+        raise SystemExit("ncu failed: " + r.stderr[-2000:])
+    rows = list(csv.reader(io.StringIO(r.stdout)))
+    hdr, units, launches = rows[0], rows[1], rows[2:]
+
+    def col(name, scale_units):
+        i = hdr.index(name)
+        return [float(l[i]) * scale_units.get(units[i], 1.0) for l in launches]
+    byte_units = {"byte": 1.0, "Kbyte": 1e3, "Mbyte": 1e6, "Gbyte": 1e9, "Tbyte": 1e12}
+    dram = [a + b for a, b in zip(col("dram__bytes_read.sum", byte_units), col("dram__bytes_write.sum", byte_units))]
+    tinst = sum(col("smsp__thread_inst_executed.sum", {}))
+    ms = col("gpu__time_duration.sum", {"ns": 1e-6, "us": 1e-3, "ms": 1.0, "s": 1e3})
+    try:
+        db = json.load(open(out_json))
+    except Exception:
+        db = {}
+    if db.get("source_hash") != kernel_source_hash():
+        db = {"source_hash": kernel_source_hash(), "entries": {}}
+    db["note"] = ("ncu figures bench.py quotes (never measured inside the timed run); valid only for the kernel sources with this hash "
+                  "(paper_2606_23698_b200.ledger.kernel_source_hash), otherwise bench.py prints null")
+    db["entries"][key] = {"dram_bytes_per_launch": sum(dram) / len(dram), "dram_bytes_per_launch_each": dram,
+                          "thread_inst_per_output_eq": tinst / n_out, "launches": len(launches), "ncu_ms_per_launch": ms,
+                          "n_out": n_out, "command": command}
+    json.dump(db, open(out_json, "w"), indent=1)
+    return json.dumps(db["entries"][key], indent=1)
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("report", nargs="?")
@@ -214,12 +290,24 @@ def main():
     ap.add_argument("--md", help="write the tables to this file as well")
     ap.add_argument("--lines", help="write the per-line counts (file, line, term, thread inst, predicated-on) as CSV")
     ap.add_argument("--launch", type=int, default=0, help="index of the launch to read in a report that holds several (default 0)")
+    ap.add_argument("--summary", action="store_true", help="key raw metrics of every launch in the report (no --n-out needed)")
+    ap.add_argument("--constants", help="write / update this JSON (profiles/ncu_constants.json) from a report holding every stage launch of one transform")
+    ap.add_argument("--key", help="entry name for --constants: VARIANT:SIZE, e.g. bf:1024 or bf-unfused:1024")
+    ap.add_argument("--command", default="", help="the ncu command that made the report (recorded with --constants)")
     ap.add_argument("--static", action="store_true", help="SASS opcode histogram of libozfft.so (no report needed)")
     a = ap.parse_args()
     global LAUNCH
     LAUNCH = a.launch
     if a.static:
         out = static_histogram(os.path.join(_HERE, "libozfft.so"))
+    elif a.constants:
+        if not (a.report and a.n_out and a.key):
+            ap.error("REPORT, --n-out and --key are required with --constants")
+        out = constants(a.report, a.key, a.n_out, a.constants, a.command)
+    elif a.summary:
+        if not a.report:
+            ap.error("REPORT is required")
+        out = summary(a.report)
     else:
         if not a.report or not a.n_out:
             ap.error("REPORT and --n-out are required")

@@ -2,17 +2,18 @@
 fused -- both stages of an axis of length 1024 in one launch, Y' in an L2-resident ring -- and unfused (two launches per
 axis, OZFFT_SCHEDULE=unfused).  Both must equal the oracle bit for bit.  The shapes cover: the contiguous axis fused
 (ring [k2][pencil][j1]), a strided axis fused (ring [k2][j1][lane]), the strided axis that also takes the z permutation
-out (8 x 16 patch, p = 8 and p = 32), more groups than ring slots (slot reuse, both hand-shakes), a fused axis next to an
+out (8 x 16 patch), more groups than ring slots (slot reuse, both hand-shakes), a fused axis next to an
 unfusable one (inner length 2), and the batched 1-D plan."""
 import numpy as np
 import pytest
 
 pytestmark = pytest.mark.gpu
 
-SHAPES = [((8, 64, 1024), 5, 4),     # z fused (4 groups), y two unfused stages with the patch (p = 32)
+SHAPES = [((8, 64, 1024), 5, 4),     # z fused (4 groups, output permuted along z), y two unfused stages, the first with the patch
           ((1024, 4, 128), 6, 4),    # x fused (strided, 4 groups)
-          ((2, 1024, 256), 7, 4),    # y fused AND un-permuting (patch, p = 8); z permuted (nz = 256)
-          ((8, 256, 1024), 8, 4),    # z fused with 16 groups > 14 ring slots
+          ((2, 1024, 256), 7, 4),    # y fused (2 groups); z of length 256 keeps the natural order
+          ((2, 1024, 1024), 11, 3),  # z fused and permuted, y fused AND un-permuting (patch)
+          ((16, 256, 1024), 8, 4),    # z fused with 32 groups > 16 ring slots
           ((1024, 1024, 2), 9, 4)]   # x fused, y cannot be (inner length 2)
 
 
