@@ -87,6 +87,10 @@ int ozfft_probe_cp(int kbytes, const void *dA, void *dD, void *stream);
  * Synchronises `stream`.  Device pointers. */
 int ozfft_probe_crt(int n, const void *d_residues, void *d_out, int variant, void *stream);
 
+/* Host-only: block `block` (32 tiles) of the fused-axis tile sequence for `groups` groups and lag `lag` (csrc/stage_bf.cuh
+ * bf_sequence, the function the kernel uses) -> *stage (0 first, 1 second), *group.  The plan uses lag = min(8, groups) and a
+ * ring of 16 slots.  Returns OZFFT_OK or OZFFT_EINVAL. */
+int ozfft_debug_fuse_sequence(int block, int lag, int groups, int *stage, int *group);
 /* Pipeline timers of the byte-fed stage kernel (measuring build only: paper_2606_23698_b200/build.py --timers compiles with
  * -DOZFFT_PIPE_TIMERS; the product build returns 0 and writes nothing).  h receives 160 x 12 uint64 (HOST pointer), one row per
  * CTA of the LAST launch, in SM clock cycles summed over the CTA's tiles: [0] issuer waiting for the data operand (a_full),

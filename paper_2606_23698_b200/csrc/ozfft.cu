@@ -692,6 +692,12 @@ int ozfft_debug_timers(unsigned long long *h) {
 #endif
 }
 
+int ozfft_debug_fuse_sequence(int block, int lag, int groups, int *stage, int *group) {
+    if (block < 0 || groups < 1 || lag < 1 || lag > groups || block >= 2 * groups || !stage || !group) return OZFFT_EINVAL;
+    bf_sequence(block, lag, groups, *stage, *group);
+    return OZFFT_OK;
+}
+
 uint64_t ozfft_twiddle_checksum(void) { return twiddle_fnv(twiddles()); }
 
 int ozfft_plan_num_launches(ozfft_plan p) { return valid(p) ? (int)p->stages.size() : -1; }

@@ -211,6 +211,17 @@ constexpr unsigned BF_RD_TARGET = 32 * 8;          // second-stage tiles x decon
 
 struct BfLoc { int st, grp, tl, tbi, tsi, toi, tbo, tso, too; };
 
+// block q (32 tiles) of the fused tile sequence -> (stage, group): the first-stage blocks of the first Lg groups, then
+// alternately the first stage of group Lg + i and the second stage of group i, then the second-stage blocks of the last Lg
+// groups.  tests/test_fuse_sequence_cpu.py checks on the host that this is a bijection and that every wait of the ring
+// hand-shake points at earlier blocks.
+__host__ __device__ inline void bf_sequence(int q, int Lg, int G, int &st, int &grp) {
+    if (q < Lg) { st = 0; grp = q; return; }
+    const int r = q - Lg;
+    if (r < 2 * (G - Lg)) { st = r & 1; grp = st ? (r >> 1) : Lg + (r >> 1); }
+    else { st = 1; grp = G - Lg + (r - 2 * (G - Lg)); }
+}
+
 template <bool FUSED>
 __device__ __forceinline__ BfLoc bf_locate(const StageGeom &g, const BfFuse &f, long long tile, int lg_nbt, int lg_ns) {
     BfLoc L;
@@ -221,14 +232,8 @@ __device__ __forceinline__ BfLoc bf_locate(const StageGeom &g, const BfFuse &f, 
         L.tbi = L.tbo = tb; L.tsi = L.tso = ts; L.toi = L.too = to;
         return L;
     }
-    const int q = (int)(tile >> 5), Lg = f.Lg, G = f.G;
     L.tl = (int)tile & 31;
-    if (q < Lg) { L.st = 0; L.grp = q; }
-    else {
-        const int r = q - Lg;
-        if (r < 2 * (G - Lg)) { L.st = r & 1; L.grp = L.st ? (r >> 1) : Lg + (r >> 1); }
-        else { L.st = 1; L.grp = G - Lg + (r - 2 * (G - Lg)); }
-    }
+    bf_sequence((int)(tile >> 5), f.Lg, f.G, L.st, L.grp);
     const int gb = L.grp & ((1 << f.lg_nbt) - 1), go = L.grp >> f.lg_nbt;
     if (L.st == 0) { L.tbi = gb * f.s1_mulb + L.tl * f.s1_tlb; L.tsi = L.tl * f.s1_tls; L.toi = go; L.tbo = L.tl * f.r1_tlb; L.tso = L.tl * f.r1_tls; L.too = 0; }
     else { L.tbi = 0; L.tsi = L.tl; L.toi = 0; L.tbo = gb; L.tso = L.tl; L.too = go; }
@@ -242,6 +247,7 @@ template <bool FUSED> __device__ __forceinline__ uint4 bf_ld(const uint4 *p) {
     asm volatile("ld.global.cg.v4.u32 {%0,%1,%2,%3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "l"(p));
     return v;
 }
+// [ledger: sync: fused-axis ring counters (global acquire polls)]
 // wait until a global counter reaches `target` (acquire; bounded: a protocol bug must trap, not hang)
 __device__ __forceinline__ void bf_wait_global(const unsigned int *ctr, unsigned int target) {
     unsigned int v, spins = 0;

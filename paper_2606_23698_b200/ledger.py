@@ -86,10 +86,16 @@ def _ncu(args):
 
 
 def read_lines(report):
-    """[(file, line, thread_inst, pred_on_thread_inst)] per source line and [(opcode, thread_inst)] per SASS instruction"""
+    """[(file, line, thread_inst, pred_on_thread_inst)] per source line and [(opcode, thread_inst)] per SASS instruction.
+    The source page lists an inlined instruction under EVERY frame of its inline stack (call site, wrapper, callee line):
+    each SASS address is counted once, under the innermost frame -- taken to be the listing line with the smallest
+    aggregate, the most specific one."""
     rows = list(csv.reader(io.StringIO(_ncu(["-i", report, "--page", "source", "--csv", "--print-source", "sass,cuda"]))))
-    per = collections.OrderedDict()
     f = None
+    cur = None
+    agg = {}                                  # (file, line) -> aggregate thread inst of the listing line
+    seen = collections.defaultdict(list)      # address -> [(file, line)]
+    own = {}                                  # address -> (thread inst, pred-on thread inst)
     for r in rows:
         if not r:
             continue
@@ -97,14 +103,25 @@ def read_lines(report):
             f = os.path.basename(r[1])
         elif r[0] == "Line No" and len(r) > 8:
             h = r
-            it, ip, il = h.index("Thread Instructions Executed"), h.index("Predicated-On Thread Instructions Executed"), h.index("Line No")
-        elif f and r[0] not in ("Function Name",) and len(r) > 8 and r[il].strip():
-            try:
-                key = (f, int(r[il]))
-                a, b = per.get(key, (0, 0))
-                per[key] = (a + int(r[it]), b + int(r[ip]))
-            except ValueError:
-                pass
+            it, ip, il, ia = h.index("Thread Instructions Executed"), h.index("Predicated-On Thread Instructions Executed"), h.index("Line No"), h.index("Address")
+        elif f and r[0] not in ("Function Name",) and len(r) > 8:
+            if r[il].strip():
+                try:
+                    cur = (f, int(r[il]))
+                    agg[cur] = agg.get(cur, 0) + int(r[it])
+                except ValueError:
+                    cur = None
+            elif cur and r[ia].startswith("0x"):
+                try:
+                    own[r[ia]] = (int(r[it]), int(r[ip]))
+                    seen[r[ia]].append(cur)
+                except ValueError:
+                    pass
+    per = collections.OrderedDict()
+    for addr, places in seen.items():
+        key = min(places, key=lambda k: agg.get(k, 0))
+        a, b = per.get(key, (0, 0))
+        per[key] = (a + own[addr][0], b + own[addr][1])
     ops = collections.Counter()
     rows = list(csv.reader(io.StringIO(_ncu(["-i", report, "--page", "source", "--csv", "--print-source", "sass"]))))
     hdr = None
@@ -147,6 +164,10 @@ def report(path, n_out, moduli=12):
     o = []
     o.append(f"kernel: {raw.get('Kernel Name', '?')}  grid {raw.get('Grid Size', '?')}  duration {raw.get('gpu__time_duration.sum', '?')} ms")
     o.append(f"n_out (output-equivalents of the launch) = {n_out:.0f}")
+    o.append("")
+    o.append("Per-line counts come from ncu's instrumented replay (REPORT must hold ONE launch): the arithmetic terms are exact, but the kernel "
+             "runs slower under instrumentation, so its waiting roles spin longer and the two `sync` terms are inflated; the un-instrumented "
+             "total is the last line (warp instructions x 32 / n_out, hardware counter), and total minus the arithmetic terms is the real polling.")
     o.append("")
     o.append("| term (SURVEY.md 8(a)) | thread inst / output-eq | predicated-on | share |")
     o.append("|---|---|---|---|")
@@ -253,7 +274,7 @@ def kernel_source_hash():
 
 def constants(report, key, n_out, out_json, command):
     """profiles/ncu_constants.json entry `key` (e.g. "bf:1024") from a report that holds ALL stage launches of one transform:
-    DRAM bytes per launch (mean), thread instructions per output-equivalent (sum over the launches / n_out)."""
+    DRAM bytes per launch (mean), thread instructions per output-equivalent (32 x warp instructions summed over the launches / n_out)."""
     import json
     r = subprocess.run(["ncu", "-i", report, "--page", "raw", "--csv"], capture_output=True, text=True)
     if r.returncode != 0:
@@ -266,7 +287,7 @@ def constants(report, key, n_out, out_json, command):
         return [float(l[i]) * scale_units.get(units[i], 1.0) for l in launches]
     byte_units = {"byte": 1.0, "Kbyte": 1e3, "Mbyte": 1e6, "Gbyte": 1e9, "Tbyte": 1e12}
     dram = [a + b for a, b in zip(col("dram__bytes_read.sum", byte_units), col("dram__bytes_write.sum", byte_units))]
-    tinst = sum(col("smsp__thread_inst_executed.sum", {}))
+    tinst = 32.0 * sum(col("smsp__inst_executed.sum", {}))  # warp instructions x 32: issue-slot equivalents (predicated-off lanes included)
     ms = col("gpu__time_duration.sum", {"ns": 1e-6, "us": 1e-3, "ms": 1.0, "s": 1e3})
     try:
         db = json.load(open(out_json))

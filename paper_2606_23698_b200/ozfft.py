@@ -12,7 +12,7 @@ _lib = None
 
 SYMBOLS = ["ozfft_plan_create", "ozfft_plan_create_1d", "ozfft_exec", "ozfft_exec_host", "ozfft_plan_destroy",
            "ozfft_last_error", "ozfft_twiddle_checksum", "ozfft_plan_num_launches", "ozfft_plan_device_bytes",
-           "ozfft_exec_axis", "ozfft_probe_mma", "ozfft_probe_chain", "ozfft_probe_crt", "ozfft_debug_bf_tables", "ozfft_probe_cp", "ozfft_debug_timers"]
+           "ozfft_exec_axis", "ozfft_probe_mma", "ozfft_probe_chain", "ozfft_probe_crt", "ozfft_debug_bf_tables", "ozfft_probe_cp", "ozfft_debug_timers", "ozfft_debug_fuse_sequence"]
 
 
 def lib():
@@ -41,6 +41,7 @@ def lib():
         L.ozfft_probe_crt.argtypes = [C.c_int, vp, vp, C.c_int, vp]
         L.ozfft_probe_cp.argtypes = [C.c_int, vp, vp, vp]
         L.ozfft_debug_timers.argtypes = [vp]
+        L.ozfft_debug_fuse_sequence.argtypes = [C.c_int, C.c_int, C.c_int, C.POINTER(C.c_int), C.POINTER(C.c_int)]
         L.ozfft_debug_bf_tables.restype = C.c_size_t
         L.ozfft_debug_bf_tables.argtypes = [C.c_int, C.c_int, C.c_int, vp, vp, vp]
         _lib = L
