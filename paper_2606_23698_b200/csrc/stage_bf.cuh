@@ -432,9 +432,9 @@ __global__ void __launch_bounds__(BF_THREADS, 1) stage_bf_kernel(StageGeom g, co
         // ------------------------------------------------ deconstruction: thread = (column, parity of j)
         const int dw = warp - 4, par = lane >> 4, c = dw * 16 + (lane & 15);
         constexpr int BS = H < 8 ? H : 8;  // elements loaded together (memory-level parallelism)
-        // this thread's column offset: kept across tiles in the two-launch kernel (every per-tile instruction counts at this
-        // utilisation: -13 % at 512^3); recomputed per tile in the fused kernel, where two more 64-bit values would spill
-        const long long cin1 = FUSED ? 0 : col_part(g.ci, c);
+        // this thread's column offsets (either stage), kept across tiles as 32-bit values (they are below 2^22 for every plan):
+        // every per-tile, per-thread instruction counts at this utilisation (-13 % at 512^3, -3 % at 1024^3 fused)
+        const int cin1 = (int)col_part(g.ci, c), cin2 = FUSED ? (int)col_part(f.g2.ci, c) : 0;
         uint32_t it = 0;
 #ifdef OZFFT_PIPE_TIMERS
         long long dbg_[12] = {0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0};
@@ -447,8 +447,8 @@ __global__ void __launch_bounds__(BF_THREADS, 1) stage_bf_kernel(StageGeom g, co
             const bool valid = FUSED || L.tbi * BF_COLS + c < g.ncols;
             const long long ji = second ? f.g2.ji : g.ji;
             const uint4 *src = second
-                ? f.ring + ((long long)(L.grp & (f.R - 1)) * BF_GROUP_ELEMS + col_off(f.g2.ci, L.tbi, c) + (long long)L.tsi * f.g2.is + (long long)par * ji)
-                : in + (tile_part(g.ci, L.tbi) + (FUSED ? col_part(g.ci, c) : cin1) + (long long)L.tsi * g.is + (long long)L.toi * g.io + (long long)par * ji);
+                ? f.ring + ((long long)(L.grp & (f.R - 1)) * BF_GROUP_ELEMS + tile_part(f.g2.ci, L.tbi) + cin2 + (long long)L.tsi * f.g2.is + (long long)par * ji)
+                : in + (tile_part(g.ci, L.tbi) + cin1 + (long long)L.tsi * g.is + (long long)L.toi * g.io + (long long)par * ji);
             const long long jstep = 2 * ji;
             if (FUSED) {  // the ring hand-shake (see BfFuse): data of this group written / the slot to be overwritten read
                 OZ_T0();
@@ -556,7 +556,7 @@ __global__ void __launch_bounds__(BF_THREADS, 1) stage_bf_kernel(StageGeom g, co
         const long long tstart_ = clock64();
 #endif
         int turn = qd;            // units to skip until the next one of this group (units go round-robin over the groups)
-        const long long cout1 = FUSED ? 0 : col_part(g.co, row);
+        const int cout1 = (int)col_part(g.co, row), cout2 = FUSED ? (int)col_part(f.g2.co, row) : 0;
         unsigned int wr_cnt = 0;  // fused axis: units of a first-stage tile this warp has stored and not yet counted
         int wr_grp = 0;
         for (long long tile; (tile = bf_tile(it)) < ntiles; it++) {
@@ -571,8 +571,8 @@ __global__ void __launch_bounds__(BF_THREADS, 1) stage_bf_kernel(StageGeom g, co
             const bool second = FUSED && L.st;
             const bool valid = FUSED || L.tbo * BF_COLS + row < g.ncols;
             const long long ko = second ? f.g2.ko : g.ko;
-            uint4 *dstp = second ? out + (col_off(f.g2.co, L.tbo, row) + (long long)L.tso * f.g2.os + (long long)L.too * f.g2.oo)
-                          : (FUSED ? f.ring + (long long)(L.grp & (f.R - 1)) * BF_GROUP_ELEMS : out) + (tile_part(g.co, L.tbo) + (FUSED ? col_part(g.co, row) : cout1) + (long long)L.tso * g.os + (long long)L.too * g.oo);
+            uint4 *dstp = second ? out + (tile_part(f.g2.co, L.tbo) + cout2 + (long long)L.tso * f.g2.os + (long long)L.too * f.g2.oo)
+                          : (FUSED ? f.ring + (long long)(L.grp & (f.R - 1)) * BF_GROUP_ELEMS : out) + (tile_part(g.co, L.tbo) + cout1 + (long long)L.tso * g.os + (long long)L.too * g.oo);
             const uint4 *ct = second ? f.ctab2 + (size_t)L.tso * K : ctab + (size_t)((!FUSED && g.matsel) ? L.tso : 0) * K;
             { OZ_T0(); bf_wait_slack(&a_full[0], it & 1); OZ_T1(6); }  // the column exponents of this tile are published (s_T is double buffered: the
             const int Tmax = s_T[buf][row], flag = s_flag[buf][row];  // deconstruction runs at most one tile ahead)
