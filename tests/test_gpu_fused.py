@@ -76,3 +76,33 @@ def test_axis_hook_matches_fused_transform(schedule):
     torch.cuda.synchronize()
     plan.destroy()
     assert torch.equal(full.view(torch.float64), cur.view(torch.float64))
+
+
+def test_edge_columns_through_the_fused_axis(O, schedule):
+    """all-zero, subnormal, huge, DC, impulse, wide-exponent and non-finite pencils in a batch that takes the fused schedule
+    (256 pencils = 2 groups): exact zeros and tiny results go through the generic pack, zero / non-finite columns through the
+    flag path of both stages, and every group counter still reaches its target."""
+    import torch
+    from paper_2606_23698_b200 import ozfft
+    rng = np.random.default_rng(3)
+    x = (rng.standard_normal((256, 1024)) + 1j * rng.standard_normal((256, 1024)))
+    x[0] = 0
+    x[1] *= 5e-324 * 1e3
+    x[2] *= 1e300
+    x[3, ::2] = 0
+    x[4] = 1.0
+    x[5] = 0; x[5, 0] = 1.0
+    x[6].real = np.ldexp(1.0, -rng.integers(0, 60, 1024)) * (1 + 2.0 ** -52)
+    e7 = rng.integers(-500, 500, 1024)
+    x[7] = np.ldexp(x[7].real, e7) + 1j * np.ldexp(x[7].imag, e7)
+    x[130, 77] = np.inf
+    x[200] = 0
+    plan = ozfft.Plan.batched_1d(1024, 256)
+    assert plan.num_launches == (1 if schedule == "fused" else 2)
+    got = plan.exec(torch.from_numpy(x).cuda()).cpu().numpy()
+    plan.destroy()
+    want = O.fft1d(x, -1, route=0)[0]
+    assert np.array_equal(_bits(got), _bits(want))
+    assert got[4, 0] == 1024 and np.all(got[4, 1:] == 0)
+    assert np.all(got[5] == 1.0)
+    assert np.isnan(got[130]).all() and not np.isnan(got[129]).any()
