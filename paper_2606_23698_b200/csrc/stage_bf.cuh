@@ -126,10 +126,11 @@ inline void build_pa_bf(uint8_t *pa, const CrtConsts &C) {
 
 
 // ---------------------------------------------------------------------------------------------------- kernel
-// Warp roles (768 threads): warp 0 = matrix producer (TMA bulk copies into a ring), warp 1 = stage MMA issuer,
-// warp 2 = Phase-A MMA issuer, warp 3 idle, warps 4-11 = deconstruction (a1-a3: load, column exponent, quantise, byte planes),
-// warps 12-23 = epilogue (a7-a9, a12: deposits, lift, pack, store; three groups of four warps, one TMEM lane
-// quarter each).  All hand-offs are mbarriers; there is no block-wide barrier inside the tile loop.
+// Warp roles (768 threads): warp 0 = matrix producer (TMA bulk copies into a ring), warp 1 = the one tensor-core issuer
+// (tcgen05.cp, stage MMAs, Phase-A MMAs: program order is execution order), warps 2-3 idle, warps 4-11 = deconstruction
+// (a1-a3: load, column exponent, quantise, byte planes), warps 12-23 = epilogue (a7-a9, a12: deposits, lift, pack, store;
+// three groups of four warps, one TMEM lane quarter each).  All hand-offs are mbarriers; there is no block-wide barrier
+// inside the tile loop.  One CTA per SM: 488 of the 512 TMEM columns, 178 KB of shared memory, 80 registers per thread.
 constexpr int BF_NG = 3;            // epilogue groups of four warps (units go round-robin over them)
 constexpr int BF_THREADS = 128 * (3 + BF_NG);
 constexpr int BF_NSLOT = 8;         // matrix ring: half-slots of one parity of one chunk; a ring entry is one chunk (two of them)
@@ -150,10 +151,10 @@ __device__ unsigned long long g_bf_dbg[160][12];  // per CTA: see ozfft_debug_ti
 #define OZ_T1(i)
 #endif
 // [ledger: sync: mbarrier waits]
-// bounded wait: a pipeline bug must not hang the GPU (traps after 2^26 failed polls).  The poll loop is four
-// instructions; BACKOFF > 0 parks the warp that many nanoseconds between polls (roles with slack: their polls would
-// otherwise take issue slots from the working warps).
-template <int BACKOFF> __device__ __forceinline__ void bf_wait_t(uint64_t *bar, uint32_t parity) {
+// bounded wait: a pipeline bug must not hang the GPU (traps after 2^26 failed polls).  Measured and left alone: dropping the
+// poll counter (a tighter loop) costs 9 % at 1024^3, a nanosleep or a short arithmetic delay between polls 0.5-1.5 %, back-off
+// only on the waits with slack nothing -- the loop below is the best of the forms tried.
+template <int UNUSED> __device__ __forceinline__ void bf_wait_t(uint64_t *bar, uint32_t parity) {
     const uint32_t a = smem_u32(bar);
     uint32_t done, spins = 0;
     do {
@@ -295,9 +296,8 @@ __global__ void __launch_bounds__(BF_THREADS, 1) stage_bf_kernel(StageGeom g, co
     const uint32_t tmem = s_tmem;
     if (tmem != 0) __trap();  // the CTA owns all 512 columns of its SM: the allocation starts at lane 0, column 0
 
-    // register budget per role (setmaxnreg, per warpgroup): control 32, deconstruction 80, epilogue 64 (the launch value)
-    // slot uses of the matrix ring per tile and per slot: with an even number of uses per slot and tile (K = 32) every
-    // ring index and barrier parity below is a compile-time constant after unrolling
+    // uses of a matrix ring entry per tile: the chunk loops below are unrolled once around the ring, so every ring index is a
+    // compile-time constant
     constexpr int UPT = (NCH + BF_NCS - 1) / BF_NCS;
     static_assert(NCH <= BF_NCS || NCH % BF_NCS == 0, "matrix ring: chunks per tile must tile the ring");
     if (warp == 0) {
