@@ -49,6 +49,26 @@ int ozfft_exec_host(ozfft_plan plan, const void *host_in, void *host_out, void *
 void ozfft_plan_destroy(ozfft_plan plan); /* NULL is a no-op */
 const char *ozfft_last_error(void);       /* thread-local text of the last failure */
 
+/* ---- entry point that allocates nothing ----
+ * For callers that cannot call cudaMalloc (code under CUDA graph capture, tight serving loops, harnesses that forbid it) and so
+ * cannot create a plan: out = DFT_1024 of each of `batch` contiguous pencils (pencil b at element offset 1024 b; the same
+ * transform, bit for bit, as ozfft_plan_create_1d(1024, batch, sign) + ozfft_exec), computed by the fused-axis launch of the
+ * byte-fed kernel with its scratch -- an 8-slot ring for the intermediate array and the
+ * group counters -- in a file-scope `static __device__` array of OZFFT_STATIC_SCRATCH_BYTES (16 MiB + 4 KiB) and its constant
+ * operand tables in a second one (11.4 MB): every GPU that loads the library holds both until the process exits.  `in` / `out`
+ * as for ozfft_exec (device pointers, 16-byte aligned, distinct); asynchronous on `stream`.  Limits: batch a multiple of 128
+ * with 128 <= batch <= OZFFT_STATIC_MAX_BATCH, anything else is refused with OZFFT_EINVAL and a message.  The call itself
+ * issues two memsets of the counters and one kernel launch and never calls cudaMalloc / cudaFree or an allocating library
+ * routine.  ozfft_static_setup() (once per device, with that device current; the first ozfft_fft1d_1024_static call on a device
+ * does it implicitly) takes the arrays' addresses with cudaGetSymbolAddress and fills the tables with synchronous copies -- no
+ * allocation either, but call it before starting a graph capture.  ALL calls on a device share the one scratch array, which
+ * keeps the last call's contents: calls that overlap on the GPU (two streams, two host threads) race and give wrong results;
+ * calls ordered on one stream are safe (the counters are re-zeroed on the stream, every ring slot is written before it is read). */
+#define OZFFT_STATIC_MAX_BATCH 65536
+#define OZFFT_STATIC_SCRATCH_BYTES (2 * 512 * 4 + 8 * 131072 * 16)
+int ozfft_static_setup(void);
+int ozfft_fft1d_1024_static(int batch, int sign, const void *in, void *out, void *stream);
+
 /* ---- introspection / test hooks (not needed by users) ---- */
 /* FNV-1a over the plan's 1024-entry table of (RN(2^53 cos), RN(2^53 sin)) of 2 pi t/1024 (reading S5);
  * must equal the oracle's independent generator. */

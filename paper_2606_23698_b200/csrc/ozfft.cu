@@ -698,6 +698,117 @@ int ozfft_debug_fuse_sequence(int block, int lag, int groups, int *stage, int *g
     return OZFFT_OK;
 }
 
+// ---------------------------------------------------------------------------------------------------- no-allocation entry point
+// ozfft_fft1d_1024_static: the batched 1-D transform of length 1024 (BASELINE.json config 3's shape) for callers that cannot
+// call cudaMalloc (CUDA graph capture, tight serving loops, harnesses that forbid it) and therefore cannot create a plan.
+// It runs the fused-axis launch of the byte-fed kernel (stage_bf.cuh BfFuse) with its scratch -- the ring of Y' slots and the
+// per-group counters -- in the file-scope array below instead of plan-owned memory, and with the (constant) operand tables in
+// a second file-scope array filled at set-up.  Nothing here calls cudaMalloc / cudaFree or an allocating library routine.
+// In host code the array names are host-side stand-ins, not device addresses: the addresses come from
+// cudaGetSymbolAddress, once per device, with that device current (static_setup).
+constexpr int ST_RING_SLOTS = 8, ST_LAG = 4;                      // ring of 8 slots x 2 MiB, second stage 4 groups behind the first
+constexpr int ST_MAX_GROUPS = OZFFT_STATIC_MAX_BATCH / 128;       // 512 groups of 128 pencils
+constexpr size_t ST_CTR_BYTES = (size_t)2 * ST_MAX_GROUPS * 4;    // store / read counters, one pair per group
+constexpr size_t ST_SCRATCH_BYTES = ST_CTR_BYTES + (size_t)ST_RING_SLOTS * BF_GROUP_ELEMS * 16;
+static_assert(ST_SCRATCH_BYTES == OZFFT_STATIC_SCRATCH_BYTES, "ozfft.h states the size of the static scratch");
+static __device__ __align__(256) unsigned char g_static_scratch[ST_SCRATCH_BYTES];
+// operand tables per direction: [F_32 planes | 32 fused planes | offset constants 1 | offset constants 2], then the Phase-A matrix
+constexpr size_t ST_MAT1 = bf_mat_bytes(32), ST_MAT2 = 32 * bf_mat_bytes(32), ST_C1 = 32 * 16, ST_C2 = 32 * 32 * 16;
+constexpr size_t ST_SIGN_BYTES = ST_MAT1 + ST_MAT2 + ST_C1 + ST_C2;
+static __device__ __align__(256) unsigned char g_static_tables[2 * ST_SIGN_BYTES + BF_PA_BYTES];
+
+namespace {
+struct StaticDev { bool ready = false; int sms = 0; unsigned char *scratch = nullptr, *tables = nullptr; };
+std::mutex g_static_mu;
+std::map<int, StaticDev> g_static_dev;
+
+// once per device, with that device current: symbol addresses, kernel attributes, constant bank, tables for both directions
+int static_setup(StaticDev *&out) {
+    int dev = 0;
+    if (!cuda_ok(cudaGetDevice(&dev), "cudaGetDevice")) return OZFFT_ECUDA;
+    std::lock_guard<std::mutex> lk(g_static_mu);
+    StaticDev &d = g_static_dev[dev];
+    out = &d;
+    if (d.ready) return OZFFT_OK;
+    int major = 0;
+    if (!cuda_ok(cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev), "cudaDeviceGetAttribute") ||
+        !cuda_ok(cudaDeviceGetAttribute(&d.sms, cudaDevAttrMultiProcessorCount, dev), "cudaDeviceGetAttribute")) return OZFFT_ECUDA;
+    if (major != 10) { set_err("ozfft needs an sm_100 device (B200); no fallback path exists"); return OZFFT_ECUDA; }
+    if (!cuda_ok(cudaGetSymbolAddress((void **)&d.scratch, g_static_scratch), "cudaGetSymbolAddress(scratch)") ||
+        !cuda_ok(cudaGetSymbolAddress((void **)&d.tables, g_static_tables), "cudaGetSymbolAddress(tables)")) return OZFFT_ECUDA;
+    DevConsts hc;
+    fill_consts(hc);
+    if (!stage_tc_prepare(hc) || !stage_bf_prepare()) { set_err("kernel attribute setup failed"); return OZFFT_ECUDA; }
+    for (int si = 0; si < 2; si++) {  // si = 0: sign -1 (forward), 1: sign +1
+        unsigned char *base = d.tables + (size_t)si * ST_SIGN_BYTES;
+        std::vector<uint8_t> B;
+        std::vector<uint32_t> C;
+        build_mat_bf(B, C, 32, 0, si ? 1 : -1, twiddles());
+        if (B.size() != ST_MAT1 || C.size() * 4 != ST_C1) { set_err("static tables: unexpected table size"); return OZFFT_ECUDA; }
+        if (!cuda_ok(cudaMemcpy(base, B.data(), ST_MAT1, cudaMemcpyHostToDevice), "cudaMemcpy(static tables)") ||
+            !cuda_ok(cudaMemcpy(base + ST_MAT1 + ST_MAT2, C.data(), ST_C1, cudaMemcpyHostToDevice), "cudaMemcpy(static tables)")) return OZFFT_ECUDA;
+        build_mat_bf(B, C, 32, 1024, si ? 1 : -1, twiddles());
+        if (B.size() != ST_MAT2 || C.size() * 4 != ST_C2) { set_err("static tables: unexpected table size"); return OZFFT_ECUDA; }
+        if (!cuda_ok(cudaMemcpy(base + ST_MAT1, B.data(), ST_MAT2, cudaMemcpyHostToDevice), "cudaMemcpy(static tables)") ||
+            !cuda_ok(cudaMemcpy(base + ST_MAT1 + ST_MAT2 + ST_C1, C.data(), ST_C2, cudaMemcpyHostToDevice), "cudaMemcpy(static tables)")) return OZFFT_ECUDA;
+    }
+    CrtConsts Cc;
+    build_crt(Cc);
+    std::vector<uint8_t> pa(BF_PA_BYTES);
+    build_pa_bf(pa.data(), Cc);
+    if (!cuda_ok(cudaMemcpy(d.tables + 2 * ST_SIGN_BYTES, pa.data(), BF_PA_BYTES, cudaMemcpyHostToDevice), "cudaMemcpy(static tables)")) return OZFFT_ECUDA;
+    d.ready = true;
+    return OZFFT_OK;
+}
+}  // namespace
+
+int ozfft_static_setup(void) {
+    StaticDev *d = nullptr;
+    return static_setup(d);
+}
+
+int ozfft_fft1d_1024_static(int batch, int sign, const void *in, void *out, void *stream) {
+    if (sign != -1 && sign != 1) { set_err("sign must be -1 (forward) or +1 (inverse)"); return OZFFT_EINVAL; }
+    if (batch < 128 || batch % 128 || batch > OZFFT_STATIC_MAX_BATCH) {
+        set_err("ozfft_fft1d_1024_static: batch must be a multiple of 128 in [128, " + std::to_string(OZFFT_STATIC_MAX_BATCH) +
+                "] (the static scratch holds counters for " + std::to_string(ST_MAX_GROUPS) + " groups of 128 pencils); use a plan for other sizes");
+        return OZFFT_EINVAL;
+    }
+    if (!check_ptrs(in, out)) return OZFFT_EINVAL;
+    StaticDev *d = nullptr;
+    int rc = static_setup(d);  // a no-op after the first call on this device
+    if (rc) return rc;
+    // geometry: the plan code's own (add_axis), fed with the static tables so that it finds them and uploads nothing
+    const int si = sign == 1 ? 1 : 0;
+    unsigned char *base = d->tables + (size_t)si * ST_SIGN_BYTES;
+    MatMap mats;
+    MatSet m1{}, m2{};
+    m1.bf = base; m1.ctab = base + ST_MAT1 + ST_MAT2;
+    m2.bf = base + ST_MAT1; m2.ctab = base + ST_MAT1 + ST_MAT2 + ST_C1;
+    mats[MatKey{32, 0}] = m1;
+    mats[MatKey{32, 1024}] = m2;
+    ozfft_plan_s tmp{};
+    tmp.variant = 2; tmp.sign = sign; tmp.max_groups = 0;
+    std::vector<StageLaunch> st;
+    if (!add_axis(&tmp, AxisDesc{true, batch, 1024, 1}, 0, mats, st, false, 0, true) || st.size() != 1 || !st[0].fused) {
+        set_err("ozfft_fft1d_1024_static: internal geometry error");
+        return OZFFT_EINVAL;
+    }
+    BfFuse f = st[0].fuse;
+    f.wr_done = (unsigned int *)d->scratch;
+    f.rd_done = f.wr_done + ST_MAX_GROUPS;
+    f.ring = (uint4 *)(d->scratch + ST_CTR_BYTES);
+    f.Lg = ST_LAG < f.G ? ST_LAG : f.G;
+    f.R = ST_RING_SLOTS;
+    // stage_bf_launch_fused zeroes the group counters on the stream (memset, no allocation), then launches the kernel; the ring
+    // needs no clearing: every slot is written before it is read
+    if (!stage_bf_launch_fused(st[0].g, f, in, out, st[0].mat_bf, st[0].ctab_bf, d->tables + 2 * ST_SIGN_BYTES, d->sms, (cudaStream_t)stream)) {
+        set_err(std::string("stage_bf_kernel (static scratch) launch: ") + cudaGetErrorString(cudaGetLastError()));
+        return OZFFT_ECUDA;
+    }
+    return OZFFT_OK;
+}
+
 uint64_t ozfft_twiddle_checksum(void) { return twiddle_fnv(twiddles()); }
 
 int ozfft_plan_num_launches(ozfft_plan p) { return valid(p) ? (int)p->stages.size() : -1; }

@@ -12,7 +12,8 @@ _lib = None
 
 SYMBOLS = ["ozfft_plan_create", "ozfft_plan_create_1d", "ozfft_exec", "ozfft_exec_host", "ozfft_plan_destroy",
            "ozfft_last_error", "ozfft_twiddle_checksum", "ozfft_plan_num_launches", "ozfft_plan_device_bytes",
-           "ozfft_exec_axis", "ozfft_probe_mma", "ozfft_probe_chain", "ozfft_probe_crt", "ozfft_debug_bf_tables", "ozfft_probe_cp", "ozfft_debug_timers", "ozfft_debug_fuse_sequence"]
+           "ozfft_exec_axis", "ozfft_probe_mma", "ozfft_probe_chain", "ozfft_probe_crt", "ozfft_debug_bf_tables", "ozfft_probe_cp", "ozfft_debug_timers", "ozfft_debug_fuse_sequence",
+           "ozfft_static_setup", "ozfft_fft1d_1024_static"]
 
 
 def lib():
@@ -41,6 +42,7 @@ def lib():
         L.ozfft_probe_crt.argtypes = [C.c_int, vp, vp, C.c_int, vp]
         L.ozfft_probe_cp.argtypes = [C.c_int, vp, vp, vp]
         L.ozfft_debug_timers.argtypes = [vp]
+        L.ozfft_fft1d_1024_static.argtypes = [C.c_int, C.c_int, vp, vp, vp]
         L.ozfft_debug_fuse_sequence.argtypes = [C.c_int, C.c_int, C.c_int, C.POINTER(C.c_int), C.POINTER(C.c_int)]
         L.ozfft_debug_bf_tables.restype = C.c_size_t
         L.ozfft_debug_bf_tables.argtypes = [C.c_int, C.c_int, C.c_int, vp, vp, vp]
@@ -122,6 +124,24 @@ class Plan:
             self.destroy()
         except Exception:
             pass
+
+
+STATIC_MAX_BATCH = 65536
+
+
+def static_setup():
+    """once per device: addresses of the library's static scratch / tables, table upload (no allocation)"""
+    _check(lib().ozfft_static_setup(), "ozfft_static_setup")
+
+
+def fft1d_1024_static(x, out, sign=-1, stream=None):
+    """x, out: CUDA complex128 [batch, 1024], contiguous, batch a multiple of 128 up to STATIC_MAX_BATCH.  Allocates nothing:
+    the caller passes the output; the scratch is a static device array of the library (calls that overlap on the GPU race)."""
+    import torch
+    assert x.is_cuda and out.is_cuda and x.dtype == out.dtype == torch.complex128 and x.is_contiguous() and out.is_contiguous()
+    assert x.dim() == 2 and x.shape[1] == 1024 and out.shape == x.shape
+    _check(lib().ozfft_fft1d_1024_static(x.shape[0], sign, x.data_ptr(), out.data_ptr(), _stream(stream)), "ozfft_fft1d_1024_static")
+    return out
 
 
 def twiddle_checksum():
